@@ -1,0 +1,139 @@
+/*
+ * afqmc.h -- C ABI of the B200-native batched phaseless-AFQMC local-energy library.
+ *
+ * What it computes (citations are to /root/reference/PAPER.md = arXiv 2209.04015, the ipie paper; letters
+ * follow BASELINE.json: N orbitals, n_sigma electrons of spin sigma, Ngamma Cholesky vectors, Nw walkers):
+ *
+ *   for every walker w, with a single-determinant trial psi_sigma (N x n_sigma) and walker determinants
+ *   phi_{sigma,w} (N x n_sigma, complex128):
+ *     S_sigma      = psi_sigma^dagger phi_{sigma,w}                         PAPER.md:143  (Eq. 16)
+ *     overlap      = det S_alpha * det S_beta   (returned as its logarithm)  PAPER.md:143  (Eq. 16)
+ *     theta_sigma  = (phi_{sigma,w} S_sigma^-1)^T          (n_sigma x N)     PAPER.md:191  (Eq. 23), Listing 2
+ *     E1           = sum_sigma sum_ip  htilde^sigma_ip theta^sigma_ip        PAPER.md:282, Eq. 2, Eq. 22
+ *     T^gamma_sigma= Ltilde^gamma_sigma theta_sigma^T      (n_sigma x n_sigma)  PAPER.md:239 (Eq. 29)
+ *     E            = E0 + E1 + 1/2 sum_gamma (sum_sigma Tr T^gamma_sigma)^2
+ *                            - 1/2 sum_gamma sum_sigma Tr(T^gamma_sigma T^gamma_sigma)   PAPER.md:224,234 (Eq. 26, 28)
+ *   where htilde_sigma = psi_sigma^dagger h and Ltilde^gamma_sigma = psi_sigma^dagger L^gamma are built once in
+ *   afqmc_create (Eq. 21: "only needs to be constructed once").  T is formed and consumed on chip
+ *   ("direct algorithm"); the Nw*Ngamma*n^2 tensor is never written to memory.
+ *
+ * Conventions common to all entry points
+ *   - complex128 = two float64 (re, im) interleaved; all matrices row-major; everything little-endian.
+ *   - "device" pointers are CUDA device memory of the current device; "host" pointers are ordinary (preferably
+ *     pinned) host memory.  The caller owns every buffer it passes; the library reads inputs only during the
+ *     call, writes only the named outputs, and owns its handle and internal workspaces until afqmc_destroy.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Return value: AFQMC_OK or a negative error code; afqmc_last_error() gives the text.  Argument errors are
+ *     detected before any work is enqueued.
+ *   - Requires compute capability 10.x (sm_100a); anything else returns AFQMC_ERR_ARCH.  There is no CPU path.
+ */
+#ifndef AFQMC_H_
+#define AFQMC_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct afqmc_ctx afqmc_ctx; /* opaque, library-owned */
+
+enum {
+    AFQMC_OK = 0,
+    AFQMC_ERR_ARG = -1,         /* null pointer, size out of range, n_walkers > max_walkers ...          */
+    AFQMC_ERR_ALLOC = -2,       /* cudaMalloc failed                                                    */
+    AFQMC_ERR_CUDA = -3,        /* a CUDA call or kernel launch failed                                  */
+    AFQMC_ERR_ARCH = -4,        /* device is not sm_100                                                 */
+    AFQMC_ERR_UNSUPPORTED = -5  /* valid input the library does not handle yet (complex trial, n > 64)  */
+};
+
+#define AFQMC_MAX_NOCC 64 /* largest n_sigma supported (shared-memory LU and register-tile limits) */
+
+/*
+ * afqmc_create -- one-time setup for a Hamiltonian and trial (Eq. 21).
+ *   h1e    device, float64 [N][N], real symmetric one-body matrix h_pq (Eq. 2; used as given, no shift).
+ *   chol   device, float64 [n_gamma][N][N], Cholesky vectors L^gamma_pq, each slice symmetric (Eq. 3).
+ *          Not retained: may be freed after the call returns.
+ *   trial  device, complex128: alpha block [N][n_alpha] followed by beta block [N][n_beta] (columns =
+ *          occupied orbitals; orthonormal columns expected).  The imaginary part must be
+ *          identically zero (all of BASELINE.json's configs); a complex trial returns AFQMC_ERR_UNSUPPORTED.
+ *   N >= 1; 0 <= n_alpha, n_beta <= min(N, AFQMC_MAX_NOCC); n_alpha + n_beta >= 1; n_gamma >= 1.
+ *   e0     constant energy E0 added to every walker's energy.
+ *   max_walkers >= 1 sizes the internal workspaces (theta, partial sums).
+ *   The call enqueues the half-rotation on `stream` and synchronises it before returning.
+ *   *out receives the handle (NULL on failure; on failure afqmc_last_error(NULL) holds the message).
+ */
+int afqmc_create(const double *h1e, const double *chol, const void *trial, int N, int n_alpha, int n_beta,
+                 int n_gamma, double e0, int max_walkers, void *stream, afqmc_ctx **out);
+
+/*
+ * afqmc_local_energy -- the hot path: kernels K1 (overlap, LU, inverse, theta, E1), K2 (fused exchange +
+ * Coulomb traces, once per spin) and K3 (assembly), all enqueued on `stream`; returns without synchronising.
+ *   walkers       device, complex128: alpha block [n_walkers][N][n_alpha] then beta block
+ *                 [n_walkers][N][n_beta]  ("Nwalkers x M x N").  Need not be orthonormal.
+ *   n_walkers     1 .. max_walkers.
+ *   out_energies  device, complex128 [n_walkers]: local energy E_w (Eq. 26).
+ *   out_overlaps  device, complex128 [n_walkers]: LOG-overlap, (re, im) = (log|<psi_T|phi_w>|, arg in (-pi, pi]).
+ *   A walker exactly orthogonal to the trial (zero pivot) is data, not an error: its energy is NaN+NaN i and
+ *   the real part of its log-overlap is -inf.
+ *   Outputs are valid once the caller has synchronised `stream`.  No allocation, no host copy, no host sync.
+ */
+int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out_energies,
+                       void *out_overlaps, void *stream);
+
+/*
+ * afqmc_local_energy_host -- the same computation with HOST buffers: copies `walkers_host` to an internal
+ * device buffer (cudaMemcpyAsync on `stream`), runs the kernels, copies both outputs back, and synchronises
+ * `stream` before returning.  Layouts as above.  Pinned host memory makes the copies asynchronous DMA.
+ */
+int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walkers, void *out_energies_host,
+                            void *out_overlaps_host, void *stream);
+
+/*
+ * afqmc_force_bias -- copies out the Coulomb traces of the most recent afqmc_local_energy call,
+ * xbar^gamma_w = sum_sigma Tr T^gamma_sigma = sum_pq G_pq L^gamma_pq   (Eq. 19, 24).
+ *   out  device, complex128 [n_walkers][n_gamma], n_walkers = that of the last energy call.  Enqueued on `stream`.
+ */
+int afqmc_force_bias(afqmc_ctx *ctx, void *out, void *stream);
+
+/* Frees the handle and every internal buffer.  NULL is allowed. */
+void afqmc_destroy(afqmc_ctx *ctx);
+
+/* Message of the last error on this handle (or of the last failed afqmc_create when ctx == NULL).
+ * Library-owned, valid until the next call on the same handle; never freed by the caller. */
+const char *afqmc_last_error(const afqmc_ctx *ctx);
+
+/* ---- introspection used by the benchmark and the tests (no effect on results) ------------------------- */
+
+typedef struct afqmc_info {
+    int N, n_alpha, n_beta, n_gamma, max_walkers;
+    int k_steps;           /* ceil(N/4): DMMA k-steps per output tile                                   */
+    int tile_rows[2];      /* per spin: rows (gamma,i) of the K2 CTA tile, multiple of 8                 */
+    int tile_cols[2];      /* per spin: real columns (plane,walker,j) of the K2 CTA tile, multiple of 8  */
+    int gammas_per_tile[2];
+    int walkers_per_tile[2];
+    int warps_m[2], mt[2], nt[2], stages[2], ksteps_per_chunk[2];
+    int k2_smem_bytes[2];
+    long long ltilde_bytes;   /* packed half-rotated Cholesky tensor, both spins, including padding      */
+    long long theta_bytes;    /* packed theta planes for max_walkers, both spins, including padding      */
+    long long kernel_launches; /* kernels launched by this handle so far (create + energy calls)         */
+} afqmc_info;
+
+int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info);
+
+/* Per-kernel device times of energy calls.  enable != 0 makes every later afqmc_local_energy record CUDA
+ * events around K1, K2 (both spins) and K3 on the caller's stream. */
+int afqmc_set_profiling(afqmc_ctx *ctx, int enable);
+/* After the stream has been synchronised: ms[0..2] = K1, K2, K3 of the most recent call. */
+int afqmc_last_kernel_ms(afqmc_ctx *ctx, float ms[3]);
+
+/*
+ * afqmc_fp64_peak -- register-resident FP64 throughput microbenchmark used as the roofline denominator
+ * (MEASURED_PEAKS.json has no FP64 entry).  mode 0: DMMA.8x8x4 (mma.sync m8n8k4 f64) chains;
+ * mode 1: DFMA chains.  Runs `launches` back-to-back launches on `stream`, synchronises, and writes the
+ * achieved TFLOP/s of the whole sequence to *tflops.
+ */
+int afqmc_fp64_peak(int mode, int launches, double *tflops, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFQMC_H_ */

@@ -309,3 +309,13 @@ def local_energy_batch(inp, rung: str = "auto", walkers=None, V=None):
         E[k] = r["E"]
         lo[k] = complex(r["logabs"], r["arg"])
     return E, lo
+
+
+# ----------------------------------------------------------------------------------------------
+# force bias: xbar^gamma = sum_pq G_pq L^gamma_pq        (Eq. 19)
+# ----------------------------------------------------------------------------------------------
+def force_bias(chol, psi_a, psi_b, phi_a, phi_b):
+    """xbar[gamma] from the full Green's function (no half-rotation), Eq. 19 second line."""
+    Ga, _, _ = greens_function(psi_a, phi_a)
+    Gb, _, _ = greens_function(psi_b, phi_b)
+    return np.einsum("gpq,pq->g", chol, Ga + Gb)

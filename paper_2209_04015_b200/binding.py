@@ -1,0 +1,182 @@
+"""ctypes binding with the same names as include/afqmc.h.  Argument marshalling only.
+
+PyTorch is used for device memory and streams (tensors in, tensors out); every step of the path runs in the
+library's CUDA kernels.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias", "afqmc_destroy",
+           "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_fp64_peak"]
+
+
+class AfqmcError(RuntimeError):
+    pass
+
+
+class AfqmcInfo(C.Structure):
+    _fields_ = [("N", C.c_int), ("n_alpha", C.c_int), ("n_beta", C.c_int), ("n_gamma", C.c_int),
+                ("max_walkers", C.c_int), ("k_steps", C.c_int),
+                ("tile_rows", C.c_int * 2), ("tile_cols", C.c_int * 2), ("gammas_per_tile", C.c_int * 2),
+                ("walkers_per_tile", C.c_int * 2), ("warps_m", C.c_int * 2), ("mt", C.c_int * 2), ("nt", C.c_int * 2),
+                ("stages", C.c_int * 2), ("ksteps_per_chunk", C.c_int * 2), ("k2_smem_bytes", C.c_int * 2),
+                ("ltilde_bytes", C.c_longlong), ("theta_bytes", C.c_longlong), ("kernel_launches", C.c_longlong)]
+
+
+def library_path() -> str:
+    return os.path.join(_PKG, "libafqmc.so")
+
+
+def load_library():
+    """dlopen libafqmc.so (built in-tree).  Raises if it is missing: there is no fallback path."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = library_path()
+    if not os.path.exists(path):
+        raise AfqmcError(f"{path} not found: build it first (python -c 'import __graft_entry__ as g; g.build()')")
+    lib = C.CDLL(path)
+    vp, ip, dp = C.c_void_p, C.c_int, C.c_double
+    lib.afqmc_create.argtypes = [vp, vp, vp, ip, ip, ip, ip, dp, ip, vp, C.POINTER(vp)]
+    lib.afqmc_create.restype = ip
+    lib.afqmc_local_energy.argtypes = [vp, vp, ip, vp, vp, vp]
+    lib.afqmc_local_energy.restype = ip
+    lib.afqmc_local_energy_host.argtypes = [vp, vp, ip, vp, vp, vp]
+    lib.afqmc_local_energy_host.restype = ip
+    lib.afqmc_force_bias.argtypes = [vp, vp, vp]
+    lib.afqmc_force_bias.restype = ip
+    lib.afqmc_destroy.argtypes = [vp]
+    lib.afqmc_destroy.restype = None
+    lib.afqmc_last_error.argtypes = [vp]
+    lib.afqmc_last_error.restype = C.c_char_p
+    lib.afqmc_get_info.argtypes = [vp, C.POINTER(AfqmcInfo)]
+    lib.afqmc_get_info.restype = ip
+    lib.afqmc_set_profiling.argtypes = [vp, ip]
+    lib.afqmc_set_profiling.restype = ip
+    lib.afqmc_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.afqmc_last_kernel_ms.restype = ip
+    lib.afqmc_fp64_peak.argtypes = [ip, ip, C.POINTER(dp), vp]
+    lib.afqmc_fp64_peak.restype = ip
+    _LIB = lib
+    return lib
+
+
+def _stream_ptr(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise AfqmcError("no CUDA device: this library has no CPU path")
+
+
+def fp64_peak_tflops(mode: str = "dmma", launches: int = 10) -> float:
+    """afqmc_fp64_peak: measured register-resident FP64 throughput (TFLOP/s). mode: 'dmma' | 'dfma'."""
+    _require_cuda()
+    lib = load_library()
+    out = C.c_double(0.0)
+    rc = lib.afqmc_fp64_peak(0 if mode == "dmma" else 1, launches, C.byref(out), _stream_ptr())
+    if rc != 0:
+        raise AfqmcError(f"afqmc_fp64_peak failed ({rc}): {lib.afqmc_last_error(None).decode()}")
+    return out.value
+
+
+class LocalEnergy:
+    """Handle around afqmc_create / afqmc_local_energy / afqmc_destroy.
+
+    h1e [N,N] float64, chol [Ngamma,N,N] float64, trial = complex128 vector (alpha block [N,n_alpha] then beta
+    block [N,n_beta]); all CUDA tensors.  ``chol`` is not retained.
+    """
+
+    def __init__(self, h1e, chol, trial, N, n_alpha, n_beta, n_gamma, e0, max_walkers, stream=None):
+        _require_cuda()
+        self._lib = load_library()
+        self._h = C.c_void_p(None)
+        for t, dt in ((h1e, torch.float64), (chol, torch.float64), (trial, torch.complex128)):
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == dt):
+                raise AfqmcError("inputs must be contiguous CUDA tensors of dtype float64/float64/complex128")
+        if h1e.numel() != N * N or chol.numel() != n_gamma * N * N or trial.numel() != N * (n_alpha + n_beta):
+            raise AfqmcError("input sizes do not match N, n_alpha, n_beta, n_gamma")
+        rc = self._lib.afqmc_create(h1e.data_ptr(), chol.data_ptr(), trial.data_ptr(), N, n_alpha, n_beta, n_gamma,
+                                    float(e0), max_walkers, _stream_ptr(stream), C.byref(self._h))
+        if rc != 0:
+            raise AfqmcError(f"afqmc_create failed ({rc}): {self._lib.afqmc_last_error(None).decode()}")
+        self.N, self.n_alpha, self.n_beta, self.n_gamma, self.max_walkers = N, n_alpha, n_beta, n_gamma, max_walkers
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise AfqmcError(f"{what} failed ({rc}): {self._lib.afqmc_last_error(self._h).decode()}")
+
+    def local_energy(self, walkers, n_walkers, out_energies=None, out_overlaps=None, stream=None):
+        """afqmc_local_energy on device tensors.  Returns (energies, log_overlaps) complex128 [n_walkers]."""
+        if not (walkers.is_cuda and walkers.is_contiguous() and walkers.dtype == torch.complex128):
+            raise AfqmcError("walkers must be a contiguous CUDA complex128 tensor")
+        if walkers.numel() != n_walkers * self.N * (self.n_alpha + self.n_beta):
+            raise AfqmcError("walkers has the wrong number of elements")
+        if out_energies is None:
+            out_energies = torch.empty(n_walkers, dtype=torch.complex128, device=walkers.device)
+        if out_overlaps is None:
+            out_overlaps = torch.empty(n_walkers, dtype=torch.complex128, device=walkers.device)
+        rc = self._lib.afqmc_local_energy(self._h, walkers.data_ptr(), n_walkers, out_energies.data_ptr(),
+                                          out_overlaps.data_ptr(), _stream_ptr(stream))
+        self._check(rc, "afqmc_local_energy")
+        return out_energies, out_overlaps
+
+    def local_energy_host(self, walkers_host, n_walkers, out_energies_host=None, out_overlaps_host=None, stream=None):
+        """afqmc_local_energy_host on HOST (ideally pinned) tensors; synchronises before returning."""
+        if walkers_host.is_cuda or walkers_host.dtype != torch.complex128 or not walkers_host.is_contiguous():
+            raise AfqmcError("walkers_host must be a contiguous CPU complex128 tensor")
+        if walkers_host.numel() != n_walkers * self.N * (self.n_alpha + self.n_beta):
+            raise AfqmcError("walkers_host has the wrong number of elements")
+        if out_energies_host is None:
+            out_energies_host = torch.empty(n_walkers, dtype=torch.complex128).pin_memory()
+        if out_overlaps_host is None:
+            out_overlaps_host = torch.empty(n_walkers, dtype=torch.complex128).pin_memory()
+        rc = self._lib.afqmc_local_energy_host(self._h, walkers_host.data_ptr(), n_walkers,
+                                               out_energies_host.data_ptr(), out_overlaps_host.data_ptr(),
+                                               _stream_ptr(stream))
+        self._check(rc, "afqmc_local_energy_host")
+        return out_energies_host, out_overlaps_host
+
+    def force_bias(self, n_walkers, out=None, stream=None):
+        """afqmc_force_bias: [n_walkers, n_gamma] complex128 traces of the last energy call."""
+        if out is None:
+            out = torch.empty((n_walkers, self.n_gamma), dtype=torch.complex128, device="cuda")
+        self._check(self._lib.afqmc_force_bias(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_force_bias")
+        return out
+
+    def info(self) -> dict:
+        inf = AfqmcInfo()
+        self._check(self._lib.afqmc_get_info(self._h, C.byref(inf)), "afqmc_get_info")
+        out = {}
+        for name, _ in AfqmcInfo._fields_:
+            v = getattr(inf, name)
+            out[name] = list(v) if hasattr(v, "__len__") else v
+        return out
+
+    def set_profiling(self, enable: bool):
+        self._check(self._lib.afqmc_set_profiling(self._h, int(bool(enable))), "afqmc_set_profiling")
+
+    def last_kernel_ms(self):
+        ms = (C.c_float * 3)()
+        self._check(self._lib.afqmc_last_kernel_ms(self._h, ms), "afqmc_last_kernel_ms")
+        return [float(x) for x in ms]
+
+    def close(self):
+        if self._h:
+            self._lib.afqmc_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,444 @@
+// C-ABI of the B200-native batched ph-AFQMC local-energy library (see include/afqmc.h for the contract).
+// Host logic only: argument checks, tile-shape selection, workspace ownership, kernel launches.
+// Every arithmetic step of the path runs in the kernels K0..K3 included below.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/afqmc.h"
+#include "common.cuh"
+#include "fp64_peak.cuh"
+#include "k0_setup.cuh"
+#include "k1_overlap.cuh"
+#include "k2_exchange.cuh"
+#include "k3_assemble.cuh"
+
+using namespace afqmc;
+
+namespace {
+
+constexpr int kMaxSmem = 232448;   // 227 KB opt-in dynamic shared memory per CTA on sm_100
+constexpr int kMaxAcc = 26;        // MT*NT accumulator tiles per warp (52 doubles per lane)
+
+struct SpinCfg {
+    int n = 0;
+    int MT = 0, NT = 0, WM = 0, gT = 0, wT = 0, strips = 0, ksc = 0, nchunks = 0, nstages = 0, LD = 0;
+    int n_rt = 0, n_ct_max = 0;
+    size_t k2_smem = 0, k1_smem = 0;
+    OperandLayout layA{}, layB{};
+    double *A = nullptr, *B = nullptr, *psi = nullptr, *ht = nullptr, *tbuf = nullptr, *xpart = nullptr;
+    size_t A_bytes = 0, B_bytes = 0;
+};
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct afqmc_ctx {
+    int N = 0, n_gamma = 0, maxw = 0, ksteps = 0, num_sms = 0;
+    double e0 = 0.0;
+    SpinCfg sp[2];
+    double *e1 = nullptr, *logdet = nullptr;
+    double2 *h_walkers = nullptr;      // device staging for the host-buffer entry point
+    double *h_outE = nullptr, *h_outO = nullptr;
+    int last_nw = 0;
+    long long launches = 0;
+    bool profiling = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+    std::string err;
+};
+
+namespace {
+
+int fail(afqmc_ctx *ctx, int code, const char *fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define CU_TRY(ctx, call)                                                                                   \
+    do {                                                                                                    \
+        cudaError_t e_ = (call);                                                                            \
+        if (e_ != cudaSuccess)                                                                              \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? AFQMC_ERR_ALLOC : AFQMC_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                            \
+    } while (0)
+
+size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages, int LD) {
+    size_t stage = (size_t)ksc * (strips + NT) * 256;
+    return nstages * stage + (size_t)strips * 8 * LD * 8 + (size_t)8 * NT * 4 + (size_t)K2_MAX_WT * K2_MAX_WM * 16 +
+           (size_t)2 * nstages * 8 + 16;
+}
+
+// Pick the K2 tile shape for one spin: maximise (useful rows / issued rows) x (useful cols / issued cols),
+// balanced over the 4 SM sub-partitions (strip s -> warp s % WM -> sub-partition s % 4).
+bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
+    c.n = n;
+    if (n == 0) return true;
+    const int ksteps = (N + 3) / 4;
+    double best = -1.0;
+    const int wms[3] = {12, 8, 4};
+    const double wf[3] = {1.0, 0.97, 0.85};   // measured DMMA+LDS efficiency vs resident warps (profiles/fp64_peak_r1.md)
+    for (int wT = 1; wT <= K2_MAX_WT; ++wT) {
+        const int cols = 2 * wT * n, NT = (cols + 7) / 8;
+        if (NT > 16) continue;
+        const double colEff = cols / (8.0 * NT);
+        for (int wi = 0; wi < 3; ++wi) {
+            const int WM = wms[wi];
+            for (int MT = 1; MT <= 4; ++MT) {
+                if (MT * NT > kMaxAcc) continue;
+                for (int gT = 1; gT <= n_gamma; ++gT) {
+                    const int strips = (gT * n + 7) / 8;
+                    if (strips > MT * WM) break;
+                    if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
+                    const int maxload = (strips + 3) / 4;
+                    const double rowEff = (gT * n / 8.0) / (4.0 * maxload);
+                    const int LD = (2 * n) | 1;
+                    int ksc = 4, nst = 0;
+                    for (int s = 6; s >= 3; --s)
+                        if (k2_smem_bytes(strips, NT, ksc, s, LD) <= (size_t)kMaxSmem) { nst = s; break; }
+                    if (nst == 0) {
+                        ksc = 2;
+                        for (int s = 6; s >= 3; --s)
+                            if (k2_smem_bytes(strips, NT, ksc, s, LD) <= (size_t)kMaxSmem) { nst = s; break; }
+                    }
+                    if (nst == 0) continue;
+                    const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
+                    const double fill = ntiles >= 148 ? 1.0 : ntiles / 148.0;
+                    const double lds = 1.0 - 0.03 * (double)(MT + NT) / (MT * NT);
+                    const double score = rowEff * colEff * wf[wi] * lds * (0.5 + 0.5 * fill);
+                    if (score > best + 1e-12) {
+                        best = score;
+                        c.MT = MT; c.NT = NT; c.WM = WM; c.gT = gT; c.wT = wT; c.strips = strips;
+                        c.ksc = ksc; c.nstages = nst; c.LD = LD;
+                    }
+                }
+            }
+        }
+    }
+    if (best < 0) return false;
+    c.nchunks = (ksteps + c.ksc - 1) / c.ksc;
+    c.n_rt = (n_gamma + c.gT - 1) / c.gT;
+    c.n_ct_max = (maxw + c.wT - 1) / c.wT;
+    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages, c.LD);
+    c.layA = OperandLayout{n, c.strips, ksteps, c.gT, (long long)c.strips * ksteps * 32};
+    c.layB = OperandLayout{n, c.NT, ksteps, c.wT, (long long)c.NT * ksteps * 32};
+    c.A_bytes = (size_t)c.n_rt * c.layA.tile_doubles * 8;
+    c.B_bytes = (size_t)c.n_ct_max * c.layB.tile_doubles * 8;
+    c.k1_smem = (size_t)2 * n * n * 16 + (size_t)K1_PCHUNK * n * 16 + (size_t)K1_PCHUNK * n * 8 + (size_t)n * 4 + 16;
+    return true;
+}
+
+using K2Fn = void (*)(const K2Params);
+
+template <int MT, int NT>
+K2Fn k2_pick_nt(int nt) {
+    if constexpr (NT == 0) {
+        return nullptr;
+    } else {
+        if (nt == NT) {
+            if constexpr (MT * NT <= kMaxAcc) return k2_exchange<MT, NT>;
+            else return nullptr;
+        }
+        return k2_pick_nt<MT, NT - 1>(nt);
+    }
+}
+K2Fn k2_pick(int mt, int nt) {
+    switch (mt) {
+        case 1: return k2_pick_nt<1, 16>(nt);
+        case 2: return k2_pick_nt<2, 13>(nt);
+        case 3: return k2_pick_nt<3, 8>(nt);
+        case 4: return k2_pick_nt<4, 6>(nt);
+    }
+    return nullptr;
+}
+
+void free_ctx(afqmc_ctx *c) {
+    if (!c) return;
+    for (int s = 0; s < 2; ++s) {
+        cudaFree(c->sp[s].A); cudaFree(c->sp[s].B); cudaFree(c->sp[s].psi); cudaFree(c->sp[s].ht);
+        cudaFree(c->sp[s].tbuf); cudaFree(c->sp[s].xpart);
+    }
+    cudaFree(c->e1); cudaFree(c->logdet); cudaFree(c->h_walkers); cudaFree(c->h_outE); cudaFree(c->h_outO);
+    for (auto &e : c->ev) if (e) cudaEventDestroy(e);
+    delete c;
+}
+
+int check_arch(afqmc_ctx *ctx, int *num_sms) {
+    int dev = 0;
+    CU_TRY(ctx, cudaGetDevice(&dev));
+    int major = 0, sms = 0;
+    CU_TRY(ctx, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CU_TRY(ctx, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10) return fail(ctx, AFQMC_ERR_ARCH, "device compute capability %d.x is not sm_100", major);
+    if (num_sms) *num_sms = sms;
+    return AFQMC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int afqmc_create(const double *h1e, const double *chol, const void *trial, int N, int n_alpha, int n_beta,
+                 int n_gamma, double e0, int max_walkers, void *stream_, afqmc_ctx **out) {
+    if (out) *out = nullptr;
+    if (!h1e || !chol || !trial || !out) return fail(nullptr, AFQMC_ERR_ARG, "afqmc_create: null pointer argument");
+    if (N < 1 || n_gamma < 1 || max_walkers < 1 || n_alpha < 0 || n_beta < 0 || n_alpha > N || n_beta > N ||
+        n_alpha + n_beta < 1)
+        return fail(nullptr, AFQMC_ERR_ARG, "afqmc_create: size out of range (N=%d n_alpha=%d n_beta=%d n_gamma=%d max_walkers=%d)",
+                    N, n_alpha, n_beta, n_gamma, max_walkers);
+    if (n_alpha > AFQMC_MAX_NOCC || n_beta > AFQMC_MAX_NOCC)
+        return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: n_sigma > %d is not supported yet", AFQMC_MAX_NOCC);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    int sms = 0;
+    if (int rc = check_arch(nullptr, &sms)) return rc;
+
+    afqmc_ctx *c = new afqmc_ctx();
+    c->N = N; c->n_gamma = n_gamma; c->maxw = max_walkers; c->e0 = e0; c->ksteps = (N + 3) / 4; c->num_sms = sms;
+    const int ns[2] = {n_alpha, n_beta};
+#define CR_TRY(call)                                                                                          \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess) {                                                                              \
+            int rc_ = fail(nullptr, e_ == cudaErrorMemoryAllocation ? AFQMC_ERR_ALLOC : AFQMC_ERR_CUDA,       \
+                           "afqmc_create: %s: %s", #call, cudaGetErrorString(e_));                            \
+            free_ctx(c);                                                                                      \
+            return rc_;                                                                                       \
+        }                                                                                                     \
+    } while (0)
+
+    // trial: must be real ("a real-valued array rchol"); split into per-spin real [N][n] arrays
+    const size_t ntrial = (size_t)N * (n_alpha + n_beta);
+    std::vector<double> trial_h(2 * ntrial);
+    CR_TRY(cudaMemcpyAsync(trial_h.data(), trial, 2 * ntrial * sizeof(double), cudaMemcpyDeviceToHost, stream));
+    CR_TRY(cudaStreamSynchronize(stream));
+    for (size_t k = 0; k < ntrial; ++k) {
+        if (trial_h[2 * k + 1] != 0.0 || !std::isfinite(trial_h[2 * k])) {
+            free_ctx(c);
+            return fail(nullptr, AFQMC_ERR_UNSUPPORTED,
+                        "afqmc_create: trial has a non-zero imaginary part (or a non-finite entry); complex trials are not supported yet");
+        }
+    }
+    size_t toff = 0;
+    for (int s = 0; s < 2; ++s) {
+        SpinCfg &sc = c->sp[s];
+        if (!choose_cfg(ns[s], N, n_gamma, max_walkers, sc)) {
+            free_ctx(c);
+            return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: no K2 tile shape fits n_sigma=%d", ns[s]);
+        }
+        const int n = ns[s];
+        if (n == 0) continue;
+        std::vector<double> psi_h((size_t)N * n);
+        for (size_t k = 0; k < psi_h.size(); ++k) psi_h[k] = trial_h[2 * (toff + k)];
+        toff += (size_t)N * n;
+        CR_TRY(cudaMalloc(&sc.psi, psi_h.size() * 8));
+        CR_TRY(cudaMemcpyAsync(sc.psi, psi_h.data(), psi_h.size() * 8, cudaMemcpyHostToDevice, stream));
+        CR_TRY(cudaStreamSynchronize(stream));
+        CR_TRY(cudaMalloc(&sc.ht, (size_t)n * N * 8));
+        CR_TRY(cudaMalloc(&sc.A, sc.A_bytes));
+        CR_TRY(cudaMalloc(&sc.B, sc.B_bytes));
+        CR_TRY(cudaMalloc(&sc.tbuf, (size_t)max_walkers * n_gamma * 16));
+        CR_TRY(cudaMalloc(&sc.xpart, (size_t)sc.n_rt * max_walkers * 16));
+        CR_TRY(cudaMemsetAsync(sc.A, 0, sc.A_bytes, stream));
+        CR_TRY(cudaMemsetAsync(sc.B, 0, sc.B_bytes, stream));
+        CR_TRY(cudaMemsetAsync(sc.tbuf, 0, (size_t)max_walkers * n_gamma * 16, stream));
+        k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi, N, n, sc.ht);
+        CR_TRY(cudaGetLastError());
+        dim3 grid((N + 127) / 128, n_gamma);
+        k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, sc.layA, sc.A);
+        CR_TRY(cudaGetLastError());
+        c->launches += 2;
+        K2Fn fn = k2_pick(sc.MT, sc.NT);
+        if (!fn) {
+            free_ctx(c);
+            return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: no K2 instantiation for MT=%d NT=%d", sc.MT, sc.NT);
+        }
+        CR_TRY(cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc.k2_smem));
+    }
+    size_t k1s = std::max(c->sp[0].k1_smem, c->sp[1].k1_smem);
+    CR_TRY(cudaFuncSetAttribute((const void *)k1_overlap_inverse_theta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k1s));
+    CR_TRY(cudaMalloc(&c->e1, (size_t)2 * max_walkers * 16));
+    CR_TRY(cudaMalloc(&c->logdet, (size_t)2 * max_walkers * 16));
+    CR_TRY(cudaMemsetAsync(c->e1, 0, (size_t)2 * max_walkers * 16, stream));
+    CR_TRY(cudaMemsetAsync(c->logdet, 0, (size_t)2 * max_walkers * 16, stream));
+    CR_TRY(cudaMalloc(&c->h_walkers, (size_t)max_walkers * N * (n_alpha + n_beta) * 16));
+    CR_TRY(cudaMalloc(&c->h_outE, (size_t)max_walkers * 16));
+    CR_TRY(cudaMalloc(&c->h_outO, (size_t)max_walkers * 16));
+    for (auto &e : c->ev) CR_TRY(cudaEventCreate(&e));
+    CR_TRY(cudaStreamSynchronize(stream));
+#undef CR_TRY
+    *out = c;
+    return AFQMC_OK;
+}
+
+int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out_energies, void *out_overlaps,
+                       void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!walkers || !out_energies || !out_overlaps) return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: null pointer argument");
+    if (n_walkers < 1 || n_walkers > ctx->maxw)
+        return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int N = ctx->N;
+    if (ctx->profiling) CU_TRY(ctx, cudaEventRecord(ctx->ev[0], stream));
+
+    // ---- K1 -------------------------------------------------------------------------------------------
+    K1Params p1{};
+    p1.walkers = reinterpret_cast<const double2 *>(walkers);
+    p1.n_walkers = n_walkers; p1.N = N; p1.maxw = ctx->maxw;
+    p1.spin_off[0] = 0;
+    p1.spin_off[1] = (long long)n_walkers * N * ctx->sp[0].n;
+    for (int s = 0; s < 2; ++s) {
+        p1.n[s] = ctx->sp[s].n; p1.psi[s] = ctx->sp[s].psi; p1.ht[s] = ctx->sp[s].ht;
+        p1.thetaB[s] = ctx->sp[s].B; p1.layB[s] = ctx->sp[s].layB;
+    }
+    p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
+    size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
+    k1_overlap_inverse_theta<<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    if (ctx->profiling) CU_TRY(ctx, cudaEventRecord(ctx->ev[1], stream));
+
+    // ---- K2, once per spin ------------------------------------------------------------------------------
+    for (int s = 0; s < 2; ++s) {
+        const SpinCfg &sc = ctx->sp[s];
+        if (sc.n == 0) continue;
+        K2Params p2{};
+        p2.A = sc.A; p2.B = sc.B;
+        p2.tileA_doubles = sc.layA.tile_doubles; p2.tileB_doubles = sc.layB.tile_doubles;
+        p2.n = sc.n; p2.gT = sc.gT; p2.wT = sc.wT; p2.strips = sc.strips; p2.WM = sc.WM;
+        p2.ksteps = ctx->ksteps; p2.ksc = sc.ksc; p2.nchunks = sc.nchunks; p2.nstages = sc.nstages;
+        p2.n_rt = sc.n_rt; p2.n_ct = (n_walkers + sc.wT - 1) / sc.wT;
+        p2.n_gamma = ctx->n_gamma; p2.n_walkers = n_walkers; p2.maxw = ctx->maxw; p2.LD = sc.LD;
+        p2.tbuf = sc.tbuf; p2.xpart = sc.xpart;
+        const long long ntiles = (long long)p2.n_rt * p2.n_ct;
+        const int grid = (int)std::min<long long>(ntiles, ctx->num_sms);
+        K2Fn fn = k2_pick(sc.MT, sc.NT);
+        fn<<<grid, 32 * sc.WM, sc.k2_smem, stream>>>(p2);
+        CU_TRY(ctx, cudaGetLastError());
+        ctx->launches += 1;
+    }
+    if (ctx->profiling) CU_TRY(ctx, cudaEventRecord(ctx->ev[2], stream));
+
+    // ---- K3 -------------------------------------------------------------------------------------------
+    K3Params p3{};
+    p3.n_gamma = ctx->n_gamma; p3.maxw = ctx->maxw; p3.e0 = ctx->e0;
+    for (int s = 0; s < 2; ++s) {
+        p3.n[s] = ctx->sp[s].n; p3.n_rt[s] = ctx->sp[s].n_rt; p3.tbuf[s] = ctx->sp[s].tbuf; p3.xpart[s] = ctx->sp[s].xpart;
+    }
+    p3.e1 = ctx->e1; p3.logdet = ctx->logdet;
+    p3.out_energy = reinterpret_cast<double *>(out_energies);
+    p3.out_overlap = reinterpret_cast<double *>(out_overlaps);
+    k3_assemble<<<n_walkers, K3_THREADS, 0, stream>>>(p3);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    if (ctx->profiling) { CU_TRY(ctx, cudaEventRecord(ctx->ev[3], stream)); ctx->ev_valid = true; }
+    ctx->last_nw = n_walkers;
+    return AFQMC_OK;
+}
+
+int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walkers, void *out_energies_host,
+                            void *out_overlaps_host, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!walkers_host || !out_energies_host || !out_overlaps_host)
+        return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy_host: null pointer argument");
+    if (n_walkers < 1 || n_walkers > ctx->maxw)
+        return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy_host: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t wbytes = (size_t)n_walkers * ctx->N * (ctx->sp[0].n + ctx->sp[1].n) * 16;
+    CU_TRY(ctx, cudaMemcpyAsync(ctx->h_walkers, walkers_host, wbytes, cudaMemcpyHostToDevice, stream));
+    if (int rc = afqmc_local_energy(ctx, ctx->h_walkers, n_walkers, ctx->h_outE, ctx->h_outO, stream_)) return rc;
+    CU_TRY(ctx, cudaMemcpyAsync(out_energies_host, ctx->h_outE, (size_t)n_walkers * 16, cudaMemcpyDeviceToHost, stream));
+    CU_TRY(ctx, cudaMemcpyAsync(out_overlaps_host, ctx->h_outO, (size_t)n_walkers * 16, cudaMemcpyDeviceToHost, stream));
+    CU_TRY(ctx, cudaStreamSynchronize(stream));
+    return AFQMC_OK;
+}
+
+int afqmc_force_bias(afqmc_ctx *ctx, void *out, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!out) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias: null pointer argument");
+    if (ctx->last_nw < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias: no energy call has been made on this handle");
+    const long long total = (long long)ctx->last_nw * ctx->n_gamma * 2;
+    k3_force_bias<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream_>>>(
+        ctx->last_nw, ctx->n_gamma, ctx->sp[0].n, ctx->sp[1].n, ctx->sp[0].tbuf, ctx->sp[1].tbuf, reinterpret_cast<double *>(out));
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+void afqmc_destroy(afqmc_ctx *ctx) { free_ctx(ctx); }
+
+const char *afqmc_last_error(const afqmc_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info) {
+    if (!ctx || !info) return AFQMC_ERR_ARG;
+    std::memset(info, 0, sizeof *info);
+    info->N = ctx->N; info->n_alpha = ctx->sp[0].n; info->n_beta = ctx->sp[1].n; info->n_gamma = ctx->n_gamma;
+    info->max_walkers = ctx->maxw; info->k_steps = ctx->ksteps;
+    for (int s = 0; s < 2; ++s) {
+        const SpinCfg &c = ctx->sp[s];
+        info->tile_rows[s] = c.strips * 8; info->tile_cols[s] = c.NT * 8;
+        info->gammas_per_tile[s] = c.gT; info->walkers_per_tile[s] = c.wT;
+        info->warps_m[s] = c.WM; info->mt[s] = c.MT; info->nt[s] = c.NT; info->stages[s] = c.nstages;
+        info->ksteps_per_chunk[s] = c.ksc; info->k2_smem_bytes[s] = (int)c.k2_smem;
+        info->ltilde_bytes += (long long)c.A_bytes; info->theta_bytes += (long long)c.B_bytes;
+    }
+    info->kernel_launches = ctx->launches;
+    return AFQMC_OK;
+}
+
+int afqmc_set_profiling(afqmc_ctx *ctx, int enable) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    ctx->profiling = enable != 0;
+    ctx->ev_valid = false;
+    return AFQMC_OK;
+}
+
+int afqmc_last_kernel_ms(afqmc_ctx *ctx, float ms[3]) {
+    if (!ctx || !ms) return AFQMC_ERR_ARG;
+    if (!ctx->ev_valid) return fail(ctx, AFQMC_ERR_ARG, "afqmc_last_kernel_ms: profiling was not enabled for the last call");
+    for (int k = 0; k < 3; ++k) CU_TRY(ctx, cudaEventElapsedTime(&ms[k], ctx->ev[k], ctx->ev[k + 1]));
+    return AFQMC_OK;
+}
+
+int afqmc_fp64_peak(int mode, int launches, double *tflops, void *stream_) {
+    if (!tflops || launches < 1 || (mode != 0 && mode != 1)) return fail(nullptr, AFQMC_ERR_ARG, "afqmc_fp64_peak: bad argument");
+    int sms = 0;
+    if (int rc = check_arch(nullptr, &sms)) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    double *d = nullptr;
+    CU_TRY(nullptr, cudaMalloc(&d, 8));
+    cudaEvent_t e0, e1;
+    CU_TRY(nullptr, cudaEventCreate(&e0));
+    CU_TRY(nullptr, cudaEventCreate(&e1));
+    const int iters = mode == 0 ? 20000 : 50000;
+    const int threads = 512;
+    auto launch = [&]() {
+        if (mode == 0) peak_dmma<<<sms, threads, 0, stream>>>(d, iters, 1.0000001, 1e-9);
+        else peak_dfma<<<2 * sms, threads, 0, stream>>>(d, iters, 1.0000001, 1e-9);
+    };
+    launch();
+    CU_TRY(nullptr, cudaStreamSynchronize(stream));
+    CU_TRY(nullptr, cudaEventRecord(e0, stream));
+    for (int k = 0; k < launches; ++k) launch();
+    CU_TRY(nullptr, cudaEventRecord(e1, stream));
+    CU_TRY(nullptr, cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CU_TRY(nullptr, cudaEventElapsedTime(&ms, e0, e1));
+    const double flops = mode == 0 ? 2.0 * 256 * PEAK_NACC * (double)iters * (threads / 32) * sms * launches
+                                   : 2.0 * PEAK_NCH * (double)iters * threads * 2 * sms * launches;
+    *tflops = flops / (ms * 1e-3) * 1e-12;
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    return AFQMC_OK;
+}
+
+}  // extern "C"

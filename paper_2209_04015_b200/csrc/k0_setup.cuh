@@ -1,0 +1,62 @@
+// K0 -- one-time half-rotation (Eq. 21), executed by afqmc_create, not on the timed path.
+//   htilde_sigma[i][p]       = sum_q psi[q][i] h[q][p]
+//   Ltilde^gamma_sigma[i][r] = sum_p psi[p][i] L^gamma[p][r]      (real trial => real Ltilde)
+// Ltilde is written straight into K2's packed A-operand layout (common.cuh).
+#pragma once
+#include "common.cuh"
+
+namespace afqmc {
+
+// htilde: one thread per (i, p).
+__global__ void k0_half_rotate_h(const double *__restrict__ h1e, const double *__restrict__ psi,  // psi [N][n] real
+                                 int N, int n, double *__restrict__ ht /* [n][N] */) {
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n * N) return;
+    int i = idx / N, p = idx - i * N;
+    double acc = 0.0;
+    for (int q = 0; q < N; ++q) acc = fma(psi[(size_t)q * n + i], h1e[(size_t)q * N + p], acc);
+    ht[idx] = acc;
+}
+
+// Ltilde: grid = (ceil(N/128), n_gamma); thread owns one (gamma, r) and produces all i in blocks of 8.
+// psi is staged in shared memory by (p-chunk, 8 columns).
+constexpr int K0_PCHUNK = 64;
+
+__global__ void __launch_bounds__(128)
+k0_half_rotate_chol(const double *__restrict__ chol, const double *__restrict__ psi, int N, int n, int n_gamma,
+                    OperandLayout lay, double *__restrict__ packedA) {
+    __shared__ double psi_s[K0_PCHUNK * 8];  // [K0_PCHUNK][8]
+    const int g = blockIdx.y;
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const double *Lg = chol + (size_t)g * N * N;
+    const int tile = g / lay.per_tile;
+    const int row0 = (g - tile * lay.per_tile) * n;
+    for (int i0 = 0; i0 < n; i0 += 8) {
+        double acc[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k] = 0.0;
+        for (int p0 = 0; p0 < N; p0 += K0_PCHUNK) {
+            int pc = min(K0_PCHUNK, N - p0);
+            __syncthreads();
+            for (int t = threadIdx.x; t < pc * 8; t += blockDim.x) {
+                int pp = t >> 3, k = t & 7;
+                psi_s[t] = (i0 + k < n) ? psi[(size_t)(p0 + pp) * n + i0 + k] : 0.0;
+            }
+            __syncthreads();
+            if (r < N) {
+                for (int pp = 0; pp < pc; ++pp) {
+                    double l = Lg[(size_t)(p0 + pp) * N + r];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) acc[k] = fma(psi_s[pp * 8 + k], l, acc[k]);
+                }
+            }
+        }
+        if (r < N) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+                if (i0 + k < n) packedA[packed_offset(lay, tile, row0 + i0 + k, r)] = acc[k];
+        }
+    }
+}
+
+}  // namespace afqmc

@@ -1,0 +1,234 @@
+// K1 -- per (walker, spin): overlap matrix, LU with partial pivoting, log-determinant, inverse, theta, E1.
+//   S      = psi^T phi                      (n x n; real trial)              PAPER.md:143 (Eq. 16), Listing 2 line 1
+//   P S    = L U, log det S                                                   PAPER.md:146-150 ("linalg.det"), Listing 2 line 2
+//   X      = S^-1
+//   theta  = (phi X)^T  (n x N), written as separate re / im planes           PAPER.md:191 (Eq. 23), Listing 2 line 3;
+//            in K2's packed B-operand layout (common.cuh)                     re/im split: PAPER.md:260-262, 280
+//   E1     = sum_jp htilde_jp theta_jp                                        PAPER.md:282 with Eq. 2, 22
+// One CTA per (walker, spin); S and X live in shared memory for the whole kernel.
+#pragma once
+#include <math_constants.h>
+#include "common.cuh"
+
+namespace afqmc {
+
+constexpr int K1_THREADS = 256;
+constexpr int K1_PCHUNK = 32;  // rows of phi staged per pass = 8 DMMA k-steps of theta
+
+struct K1Params {
+    const double2 *walkers;       // alpha block [Nw][N][na], then beta block [Nw][N][nb]
+    int n_walkers, N, maxw;
+    int n[2];
+    long long spin_off[2];        // offset of each spin block in `walkers`, in complex elements
+    const double *psi[2];         // [N][n] real
+    const double *ht[2];          // [n][N] real
+    double *thetaB[2];            // packed B operand
+    OperandLayout layB[2];
+    double *logdet;               // [2][maxw][2]  (log|det|, arg)
+    double *e1;                   // [2][maxw][2]
+};
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+__global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params P) {
+    const int w = blockIdx.x, sp = blockIdx.y;
+    const int n = P.n[sp], N = P.N;
+    if (n == 0) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    extern __shared__ __align__(16) unsigned char k1_smem[];
+    double2 *S = reinterpret_cast<double2 *>(k1_smem);        // [n][n]
+    double2 *X = S + n * n;                                   // [n][n]
+    double2 *phis = X + n * n;                                // [K1_PCHUNK][n]
+    double *psis = reinterpret_cast<double *>(phis + K1_PCHUNK * n);  // [K1_PCHUNK][n]
+    int *perm = reinterpret_cast<int *>(psis + K1_PCHUNK * n);        // [n]
+    __shared__ int s_piv;
+    __shared__ double s_red[2 * (K1_THREADS / 32)];
+
+    const double2 *phi = P.walkers + P.spin_off[sp] + (long long)w * N * n;   // [N][n]
+    const double *psi = P.psi[sp];
+
+    // ---- S = psi^T phi ------------------------------------------------------------------------
+    for (int e = tid; e < n * n; e += K1_THREADS) S[e] = make_double2(0.0, 0.0);
+    for (int p0 = 0; p0 < N; p0 += K1_PCHUNK) {
+        const int pc = min(K1_PCHUNK, N - p0);
+        __syncthreads();
+        for (int t = tid; t < pc * n; t += K1_THREADS) {
+            phis[t] = phi[(long long)p0 * n + t];
+            psis[t] = psi[(long long)p0 * n + t];
+        }
+        __syncthreads();
+        for (int e = tid; e < n * n; e += K1_THREADS) {
+            const int i = e / n, j = e - i * n;
+            double2 acc = S[e];
+            for (int pp = 0; pp < pc; ++pp) {
+                const double a = psis[pp * n + i];
+                const double2 f = phis[pp * n + j];
+                acc.x = fma(a, f.x, acc.x);
+                acc.y = fma(a, f.y, acc.y);
+            }
+            S[e] = acc;
+        }
+    }
+    for (int e = tid; e < n; e += K1_THREADS) perm[e] = e;
+    __syncthreads();
+
+    // ---- LU with partial pivoting, in place ---------------------------------------------------------
+    double logabs = 0.0, ph_re = 1.0, ph_im = 0.0;   // meaningful on thread 0
+    bool singular = false;
+    for (int k = 0; k < n; ++k) {
+        if (warp == 0) {
+            double best = -1.0;
+            int bi = k;
+            for (int i = k + lane; i < n; i += 32) {
+                const double2 a = S[i * n + k];
+                const double m = a.x * a.x + a.y * a.y;
+                if (m > best) { best = m; bi = i; }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double m2 = __shfl_xor_sync(0xffffffffu, best, o);
+                const int i2 = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (m2 > best || (m2 == best && i2 < bi)) { best = m2; bi = i2; }
+            }
+            if (lane == 0) s_piv = bi;
+        }
+        __syncthreads();
+        const int piv = s_piv;
+        if (piv != k) {
+            for (int j = tid; j < n; j += K1_THREADS) {
+                const double2 t = S[k * n + j];
+                S[k * n + j] = S[piv * n + j];
+                S[piv * n + j] = t;
+            }
+            if (tid == 0) {
+                const int t = perm[k]; perm[k] = perm[piv]; perm[piv] = t;
+                ph_re = -ph_re; ph_im = -ph_im;
+            }
+            __syncthreads();
+        }
+        const double2 u = S[k * n + k];
+        const double m2 = u.x * u.x + u.y * u.y;
+        if (m2 == 0.0) { singular = true; break; }      // uniform: every thread reads the same u
+        const double2 inv = make_double2(u.x / m2, -u.y / m2);
+        if (tid == 0) {
+            const double au = sqrt(m2);
+            logabs += log(au);
+            const double2 ph = cmul(make_double2(ph_re, ph_im), make_double2(u.x / au, u.y / au));
+            ph_re = ph.x; ph_im = ph.y;
+        }
+        for (int i = k + 1 + tid; i < n; i += K1_THREADS) S[i * n + k] = cmul(S[i * n + k], inv);
+        __syncthreads();
+        const int m = n - k - 1;
+        for (int e = tid; e < m * m; e += K1_THREADS) {
+            const int ii = e / m;
+            const int i = k + 1 + ii, j = k + 1 + (e - ii * m);
+            const double2 l = S[i * n + k], r = S[k * n + j];
+            double2 a = S[i * n + j];
+            a.x -= l.x * r.x - l.y * r.y;
+            a.y -= l.x * r.y + l.y * r.x;
+            S[i * n + j] = a;
+        }
+        __syncthreads();
+    }
+
+    // ---- X = S^-1 : solve L U X = P -----------------------------------------------------------------
+    if (singular) {
+        for (int e = tid; e < n * n; e += K1_THREADS) X[e] = make_double2(CUDART_NAN, CUDART_NAN);
+        __syncthreads();
+    } else {
+        for (int e = tid; e < n * n; e += K1_THREADS) {
+            const int i = e / n, j = e - i * n;
+            X[e] = make_double2(perm[i] == j ? 1.0 : 0.0, 0.0);
+        }
+        __syncthreads();
+        for (int k = 0; k < n - 1; ++k) {                 // forward substitution, unit lower triangle
+            const int m = n - k - 1;
+            for (int e = tid; e < m * n; e += K1_THREADS) {
+                const int ii = e / n;
+                const int i = k + 1 + ii, j = e - ii * n;
+                const double2 l = S[i * n + k], r = X[k * n + j];
+                double2 a = X[i * n + j];
+                a.x -= l.x * r.x - l.y * r.y;
+                a.y -= l.x * r.y + l.y * r.x;
+                X[i * n + j] = a;
+            }
+            __syncthreads();
+        }
+        for (int k = n - 1; k >= 0; --k) {                // back substitution, upper triangle
+            const double2 u = S[k * n + k];
+            const double m2 = u.x * u.x + u.y * u.y;
+            const double2 inv = make_double2(u.x / m2, -u.y / m2);
+            for (int j = tid; j < n; j += K1_THREADS) X[k * n + j] = cmul(X[k * n + j], inv);
+            __syncthreads();
+            for (int e = tid; e < k * n; e += K1_THREADS) {
+                const int i = e / n, j = e - i * n;
+                const double2 l = S[i * n + k], r = X[k * n + j];
+                double2 a = X[i * n + j];
+                a.x -= l.x * r.x - l.y * r.y;
+                a.y -= l.x * r.y + l.y * r.x;
+                X[i * n + j] = a;
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- theta_jp = sum_i phi_pi X_ij ; packed write; E1 partial ----------------------------------------
+    const OperandLayout lay = P.layB[sp];
+    const int wT = lay.per_tile;
+    const int tile = w / wT, wl = w - tile * wT;
+    const int col_re = wl * n, col_im = (wT + wl) * n;
+    double *out = P.thetaB[sp];
+    const double *ht = P.ht[sp];
+    const int kk = lane & 3, jj = lane >> 2;
+    double e1r = 0.0, e1i = 0.0;
+    const int Kpad = lay.ksteps * 4;
+    for (int p0 = 0; p0 < Kpad; p0 += K1_PCHUNK) {
+        const int pc = max(0, min(K1_PCHUNK, N - p0));
+        __syncthreads();
+        for (int t = tid; t < pc * n; t += K1_THREADS) phis[t] = phi[(long long)p0 * n + t];
+        __syncthreads();
+        const int pl = warp * 4 + kk;           // 8 warps x 4 = 32 rows of the chunk
+        const int p = p0 + pl;
+        if (p < Kpad) {
+            for (int j = jj; j < n; j += 8) {
+                double2 acc = make_double2(0.0, 0.0);
+                if (p < N) {
+                    const double2 *fr = phis + pl * n;
+                    for (int i = 0; i < n; ++i) {
+                        const double2 f = fr[i], x = X[i * n + j];
+                        acc.x = fma(f.x, x.x, acc.x); acc.x = fma(-f.y, x.y, acc.x);
+                        acc.y = fma(f.x, x.y, acc.y); acc.y = fma(f.y, x.x, acc.y);
+                    }
+                    const double hv = ht[(long long)j * N + p];
+                    e1r = fma(hv, acc.x, e1r);
+                    e1i = fma(hv, acc.y, e1i);
+                }
+                out[packed_offset(lay, tile, col_re + j, p)] = acc.x;
+                out[packed_offset(lay, tile, col_im + j, p)] = acc.y;
+            }
+        }
+    }
+
+    // ---- deterministic block reduction of E1; outputs ---------------------------------------------------
+    e1r = warp_sum(e1r);
+    e1i = warp_sum(e1i);
+    if (lane == 0) { s_red[2 * warp] = e1r; s_red[2 * warp + 1] = e1i; }
+    __syncthreads();
+    if (tid == 0) {
+        double sr = 0.0, si = 0.0;
+        for (int q = 0; q < K1_THREADS / 32; ++q) { sr += s_red[2 * q]; si += s_red[2 * q + 1]; }
+        double *e1 = P.e1 + ((long long)sp * P.maxw + w) * 2;
+        double *ld = P.logdet + ((long long)sp * P.maxw + w) * 2;
+        if (singular) {
+            e1[0] = CUDART_NAN; e1[1] = CUDART_NAN;
+            ld[0] = -CUDART_INF; ld[1] = 0.0;
+        } else {
+            e1[0] = sr; e1[1] = si;
+            ld[0] = logabs; ld[1] = atan2(ph_im, ph_re);
+        }
+    }
+}
+
+}  // namespace afqmc

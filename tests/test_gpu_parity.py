@@ -1,0 +1,196 @@
+"""GPU parity: the CUDA path (through the C-ABI, via the ctypes binding) against the CPU oracle, element by
+element on the same seeded inputs.  Bar (BASELINE.json north_star): relative 1e-10 on each walker's complex
+energy and on its log-overlap."""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from gen import CONFIGS, make_inputs
+from gen.configs import Inputs
+from oracle import afqmc_oracle as orc
+
+pytestmark = pytest.mark.gpu
+RTOL = 1e-10
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_energies.json")
+
+
+def _le(inp, max_walkers=None):
+    from paper_2209_04015_b200 import LocalEnergy
+    dev = "cuda"
+    return LocalEnergy(torch.from_numpy(inp.h1e).to(dev), torch.from_numpy(inp.chol).to(dev),
+                       torch.from_numpy(inp.trial_packed()).to(dev), inp.N, inp.n_alpha, inp.n_beta, inp.n_gamma,
+                       inp.e0, max_walkers or inp.n_walkers)
+
+
+def gpu_energy(inp, le=None, idx=None):
+    own = le is None
+    le = le or _le(inp)
+    nw = inp.n_walkers if idx is None else len(idx)
+    E, lo = le.local_energy(torch.from_numpy(inp.walkers_packed(idx)).cuda(), nw)
+    torch.cuda.synchronize()
+    E, lo = E.cpu().numpy(), lo.cpu().numpy()
+    if own:
+        le.close()
+    return E, lo
+
+
+def assert_parity(E, lo, Eo, loo, tol=RTOL):
+    E, lo, Eo, loo = map(np.asarray, (E, lo, Eo, loo))
+    err = np.abs(E - Eo) / np.abs(Eo)
+    assert np.all(err <= tol), f"energy rel err max {err.max():.3e} at walker {err.argmax()}"
+    dre = np.abs(lo.real - loo.real) / np.maximum(1.0, np.abs(loo.real))
+    assert np.all(dre <= tol), f"log|ovlp| err max {dre.max():.3e}"
+    dim = np.abs((lo.imag - loo.imag + math.pi) % (2 * math.pi) - math.pi)
+    assert np.all(dim <= tol * np.maximum(1.0, np.abs(loo.real))), f"arg ovlp err max {dim.max():.3e}"
+    assert np.all(lo.imag <= math.pi) and np.all(lo.imag > -math.pi)
+
+
+# ---- small configs: every walker against the definition oracle (O1, stored ERIs) -----------------
+@pytest.mark.parametrize("name", ["tiny", "small"])
+def test_parity_all_walkers_vs_definition(name):
+    inp = make_inputs(name)
+    Eo, loo = orc.local_energy_batch(inp, rung="O1")
+    E, lo = gpu_energy(inp)
+    assert_parity(E, lo, Eo, loo)
+
+
+# ---- full-size configs, in the launch configuration bench.py times: sampled walkers ----------------
+@pytest.mark.parametrize("name", ["medium", "cu2o2", "large"])
+def test_parity_full_size_vs_golden(name):
+    """All walkers run on the GPU at BASELINE.json's full size; the sampled walkers are compared with oracle
+    values stored by tests/golden/make_golden.py (O2 = definition with streamed ERIs, O3 = Cholesky-direct),
+    and one walker is recomputed live with O3."""
+    with open(GOLDEN) as f:
+        gold = json.load(f)[name]
+    inp = make_inputs(name)
+    assert (gold["N"], gold["n_gamma"], gold["n_walkers"]) == (inp.N, inp.n_gamma, inp.n_walkers)
+    E, lo = gpu_energy(inp)
+    assert np.all(np.isfinite(E.view(np.float64))) and np.all(np.isfinite(lo.view(np.float64)))
+    for key in ("definition", "O3"):
+        if key not in gold:
+            continue
+        g = gold[key]
+        idx = g["walkers"]
+        Eo = np.array(g["E_re"]) + 1j * np.array(g["E_im"])
+        loo = np.array(g["logabs"]) + 1j * np.array(g["arg"])
+        assert_parity(E[idx], lo[idx], Eo, loo)
+    w = inp.n_walkers // 2 + 1
+    Eo, loo = orc.local_energy_batch(inp, rung="O3", walkers=[w])
+    assert_parity(E[[w]], lo[[w]], Eo, loo)
+
+
+# ---- edge cases --------------------------------------------------------------------------------------
+def _custom(seed, N, na, nb, ng, nw, noise=0.2):
+    rng = np.random.default_rng(seed)
+    a = rng.standard_normal((N, N))
+    h = 0.5 * (a + a.T) + np.diag(np.arange(N, dtype=float))
+    b = rng.standard_normal((ng, N, N))
+    chol = 0.5 * (b + b.transpose(0, 2, 1)) * np.exp(-np.arange(ng) / max(4.0, ng / 3))[:, None, None]
+    q, _ = np.linalg.qr(rng.standard_normal((N, N)))
+    psi_a = q[:, :na].astype(np.complex128)
+    q2, _ = np.linalg.qr(rng.standard_normal((N, N)))
+    psi_b = q2[:, :nb].astype(np.complex128)
+    phi_a = psi_a[None] + noise * (rng.standard_normal((nw, N, na)) + 1j * rng.standard_normal((nw, N, na)))
+    phi_b = psi_b[None] + noise * (rng.standard_normal((nw, N, nb)) + 1j * rng.standard_normal((nw, N, nb)))
+    return Inputs(name="custom", N=N, n_alpha=na, n_beta=nb, n_gamma=ng, e0=-1.25, h1e=h, chol=chol,
+                  psi_a=np.ascontiguousarray(psi_a), psi_b=np.ascontiguousarray(psi_b),
+                  phi_a=np.ascontiguousarray(phi_a), phi_b=np.ascontiguousarray(phi_b))
+
+
+@pytest.mark.parametrize("N,na,nb,ng,nw", [
+    (12, 5, 2, 9, 3),      # unequal spins, non-orthonormal walkers, odd sizes
+    (9, 4, 0, 7, 5),       # no beta electrons
+    (9, 0, 3, 7, 2),       # no alpha electrons
+    (7, 1, 1, 3, 1),       # one electron per spin, single walker
+    (33, 13, 11, 70, 7),   # ragged everything; several row tiles
+    (70, 33, 31, 41, 5),   # N not a multiple of 4, large odd n
+    (64, 64, 1, 5, 3),     # n = N = AFQMC_MAX_NOCC (theta = psi-independent limit)
+])
+def test_parity_edge_shapes(N, na, nb, ng, nw):
+    inp = _custom(100 + N, N, na, nb, ng, nw)
+    Eo, loo = orc.local_energy_batch(inp, rung="O1" if N <= 40 else "O3")
+    E, lo = gpu_energy(inp)
+    assert_parity(E, lo, Eo, loo)
+
+
+def test_fewer_walkers_than_capacity_and_ragged_tail():
+    inp = make_inputs("small", n_walkers=13)
+    le = _le(inp, max_walkers=64)
+    Eo, loo = orc.local_energy_batch(inp, rung="O3")
+    for idx in ([0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12], [3], [12, 5, 7]):
+        E, lo = gpu_energy(inp, le, idx)
+        assert_parity(E, lo, Eo[idx], loo[idx])
+    le.close()
+
+
+def test_invariance_under_column_mixing_on_gpu():
+    inp = make_inputs("small", n_walkers=4)
+    rng = np.random.default_rng(8)
+    Ca = rng.standard_normal((4, inp.n_alpha, inp.n_alpha)) + 1j * rng.standard_normal((4, inp.n_alpha, inp.n_alpha))
+    E0, lo0 = gpu_energy(inp)
+    inp2 = Inputs(**{**inp.__dict__, "phi_a": np.ascontiguousarray(inp.phi_a @ Ca)})
+    E1, lo1 = gpu_energy(inp2)
+    assert np.all(np.abs(E1 - E0) <= 1e-9 * np.abs(E0))
+    s, l = np.linalg.slogdet(Ca)
+    assert np.all(np.abs(lo1.real - lo0.real - l) < 1e-9)
+
+
+def test_singular_walker_is_data_not_error():
+    inp = make_inputs("tiny")
+    phi_a = inp.phi_a.copy()
+    phi_a[2] = 0.0           # S = 0 exactly: walker orthogonal to the trial
+    inp2 = Inputs(**{**inp.__dict__, "phi_a": phi_a})
+    E, lo = gpu_energy(inp2)
+    Eo, loo = orc.local_energy_batch(inp, rung="O3")
+    assert np.isnan(E[2].real) and np.isnan(E[2].imag) and lo[2].real == -np.inf
+    keep = [0, 1, 3]
+    assert_parity(E[keep], lo[keep], Eo[keep], loo[keep])
+
+
+def test_bitwise_determinism():
+    inp = make_inputs("small", n_walkers=16)
+    le = _le(inp)
+    E0, lo0 = gpu_energy(inp, le)
+    for _ in range(3):
+        E1, lo1 = gpu_energy(inp, le)
+        assert np.array_equal(E0.view(np.float64), E1.view(np.float64))
+        assert np.array_equal(lo0.view(np.float64), lo1.view(np.float64))
+    le.close()
+
+
+def test_host_entry_point_and_force_bias():
+    inp = make_inputs("small", n_walkers=6)
+    le = _le(inp)
+    E, lo = gpu_energy(inp, le)
+    wh = torch.from_numpy(inp.walkers_packed()).pin_memory()
+    Eh, loh = le.local_energy_host(wh, 6)
+    assert np.array_equal(Eh.numpy().view(np.float64), E.view(np.float64))
+    assert np.array_equal(loh.numpy().view(np.float64), lo.view(np.float64))
+    fb = le.force_bias(6)
+    torch.cuda.synchronize()
+    fb = fb.cpu().numpy()
+    for w in (0, 5):
+        ref = orc.force_bias(inp.chol, inp.psi_a, inp.psi_b, inp.phi_a[w], inp.phi_b[w])
+        assert np.all(np.abs(fb[w] - ref) <= 1e-10 * np.max(np.abs(ref)))
+    le.close()
+
+
+def test_errors_are_reported():
+    from paper_2209_04015_b200 import AfqmcError, LocalEnergy
+    inp = make_inputs("tiny")
+    dev = "cuda"
+    h, c = torch.from_numpy(inp.h1e).to(dev), torch.from_numpy(inp.chol).to(dev)
+    t = torch.from_numpy(inp.trial_packed()).to(dev)
+    with pytest.raises(AfqmcError, match="imaginary"):
+        LocalEnergy(h, c, t * (1 + 0.1j), inp.N, 3, 3, inp.n_gamma, 0.0, 4)
+    with pytest.raises(AfqmcError, match="out of range"):
+        LocalEnergy(h, c, t, inp.N, 3, 3, inp.n_gamma, 0.0, 0)
+    le = LocalEnergy(h, c, t, inp.N, 3, 3, inp.n_gamma, 0.0, 2)
+    w = torch.from_numpy(inp.walkers_packed()).to(dev)
+    with pytest.raises(AfqmcError):
+        le.local_energy(w, 4)
+    le.close()
