@@ -122,8 +122,11 @@ int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info);
 /* Per-kernel device times of energy calls.  enable != 0 makes every later afqmc_local_energy record CUDA
  * events around K1, K2 (both spins) and K3 on the caller's stream. */
 int afqmc_set_profiling(afqmc_ctx *ctx, int enable);
-/* After the stream has been synchronised: ms[0..2] = K1, K2, K3 of the most recent call. */
+/* After the stream has been synchronised: ms[0..2] = K1, K2 (both spins), K3 of the most recent profiled call. */
 int afqmc_last_kernel_ms(afqmc_ctx *ctx, float ms[3]);
+/* Mean of the same three times over the profiled calls since afqmc_set_profiling(ctx, 1) (the most recent
+ * 256 at most); *n_calls = how many were averaged.  The stream must have been synchronised. */
+int afqmc_mean_kernel_ms(afqmc_ctx *ctx, float ms[3], int *n_calls);
 
 /*
  * afqmc_fp64_peak -- register-resident FP64 throughput microbenchmark used as the roofline denominator

@@ -14,7 +14,8 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias", "afqmc_destroy",
-           "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_fp64_peak"]
+           "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
+           "afqmc_fp64_peak"]
 
 
 class AfqmcError(RuntimeError):
@@ -62,6 +63,8 @@ def load_library():
     lib.afqmc_set_profiling.restype = ip
     lib.afqmc_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.afqmc_last_kernel_ms.restype = ip
+    lib.afqmc_mean_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(ip)]
+    lib.afqmc_mean_kernel_ms.restype = ip
     lib.afqmc_fp64_peak.argtypes = [ip, ip, C.POINTER(dp), vp]
     lib.afqmc_fp64_peak.restype = ip
     _LIB = lib
@@ -169,6 +172,13 @@ class LocalEnergy:
         ms = (C.c_float * 3)()
         self._check(self._lib.afqmc_last_kernel_ms(self._h, ms), "afqmc_last_kernel_ms")
         return [float(x) for x in ms]
+
+    def mean_kernel_ms(self):
+        """(mean [K1, K2, K3] ms, number of profiled calls averaged)."""
+        ms = (C.c_float * 3)()
+        n = C.c_int(0)
+        self._check(self._lib.afqmc_mean_kernel_ms(self._h, ms, C.byref(n)), "afqmc_mean_kernel_ms")
+        return [float(x) for x in ms], n.value
 
     def close(self):
         if self._h:

@@ -24,6 +24,7 @@ namespace {
 
 constexpr int kMaxSmem = 232448;   // 227 KB opt-in dynamic shared memory per CTA on sm_100
 constexpr int kMaxAcc = 26;        // MT*NT accumulator tiles per warp (52 doubles per lane)
+constexpr int kProfSets = 256;     // ring of per-call event quadruples kept while profiling
 
 struct SpinCfg {
     int n = 0;
@@ -49,8 +50,8 @@ struct afqmc_ctx {
     int last_nw = 0;
     long long launches = 0;
     bool profiling = false;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
-    bool ev_valid = false;
+    std::vector<cudaEvent_t> ev;       // kProfSets x 4 events, created by the first afqmc_set_profiling(1)
+    long long prof_calls = 0;          // energy calls recorded since profiling was enabled
     std::string err;
 };
 
@@ -274,7 +275,6 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
     CR_TRY(cudaMalloc(&c->h_walkers, (size_t)max_walkers * N * (n_alpha + n_beta) * 16));
     CR_TRY(cudaMalloc(&c->h_outE, (size_t)max_walkers * 16));
     CR_TRY(cudaMalloc(&c->h_outO, (size_t)max_walkers * 16));
-    for (auto &e : c->ev) CR_TRY(cudaEventCreate(&e));
     CR_TRY(cudaStreamSynchronize(stream));
 #undef CR_TRY
     *out = c;
@@ -289,7 +289,8 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
         return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
     cudaStream_t stream = (cudaStream_t)stream_;
     const int N = ctx->N;
-    if (ctx->profiling) CU_TRY(ctx, cudaEventRecord(ctx->ev[0], stream));
+    cudaEvent_t *ev = ctx->profiling ? &ctx->ev[(size_t)(ctx->prof_calls % kProfSets) * 4] : nullptr;
+    if (ev) CU_TRY(ctx, cudaEventRecord(ev[0], stream));
 
     // ---- K1 -------------------------------------------------------------------------------------------
     K1Params p1{};
@@ -306,7 +307,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     k1_overlap_inverse_theta<<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
-    if (ctx->profiling) CU_TRY(ctx, cudaEventRecord(ctx->ev[1], stream));
+    if (ev) CU_TRY(ctx, cudaEventRecord(ev[1], stream));
 
     // ---- K2, once per spin ------------------------------------------------------------------------------
     for (int s = 0; s < 2; ++s) {
@@ -327,7 +328,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
         CU_TRY(ctx, cudaGetLastError());
         ctx->launches += 1;
     }
-    if (ctx->profiling) CU_TRY(ctx, cudaEventRecord(ctx->ev[2], stream));
+    if (ev) CU_TRY(ctx, cudaEventRecord(ev[2], stream));
 
     // ---- K3 -------------------------------------------------------------------------------------------
     K3Params p3{};
@@ -341,7 +342,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     k3_assemble<<<n_walkers, K3_THREADS, 0, stream>>>(p3);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
-    if (ctx->profiling) { CU_TRY(ctx, cudaEventRecord(ctx->ev[3], stream)); ctx->ev_valid = true; }
+    if (ev) { CU_TRY(ctx, cudaEventRecord(ev[3], stream)); ctx->prof_calls += 1; }
     ctx->last_nw = n_walkers;
     return AFQMC_OK;
 }
@@ -398,15 +399,38 @@ int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info) {
 
 int afqmc_set_profiling(afqmc_ctx *ctx, int enable) {
     if (!ctx) return AFQMC_ERR_ARG;
+    if (enable && ctx->ev.empty()) {
+        ctx->ev.assign((size_t)kProfSets * 4, nullptr);
+        for (auto &e : ctx->ev) CU_TRY(ctx, cudaEventCreate(&e));
+    }
     ctx->profiling = enable != 0;
-    ctx->ev_valid = false;
+    ctx->prof_calls = 0;
     return AFQMC_OK;
 }
 
 int afqmc_last_kernel_ms(afqmc_ctx *ctx, float ms[3]) {
     if (!ctx || !ms) return AFQMC_ERR_ARG;
-    if (!ctx->ev_valid) return fail(ctx, AFQMC_ERR_ARG, "afqmc_last_kernel_ms: profiling was not enabled for the last call");
-    for (int k = 0; k < 3; ++k) CU_TRY(ctx, cudaEventElapsedTime(&ms[k], ctx->ev[k], ctx->ev[k + 1]));
+    if (ctx->prof_calls < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_last_kernel_ms: no profiled call recorded");
+    const cudaEvent_t *ev = &ctx->ev[(size_t)((ctx->prof_calls - 1) % kProfSets) * 4];
+    for (int k = 0; k < 3; ++k) CU_TRY(ctx, cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]));
+    return AFQMC_OK;
+}
+
+int afqmc_mean_kernel_ms(afqmc_ctx *ctx, float ms[3], int *n_calls) {
+    if (!ctx || !ms || !n_calls) return AFQMC_ERR_ARG;
+    if (ctx->prof_calls < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_mean_kernel_ms: no profiled call recorded");
+    const int cnt = (int)std::min<long long>(ctx->prof_calls, kProfSets);
+    double acc[3] = {0.0, 0.0, 0.0};
+    for (int c = 0; c < cnt; ++c) {
+        const cudaEvent_t *ev = &ctx->ev[(size_t)c * 4];
+        for (int k = 0; k < 3; ++k) {
+            float t = 0.f;
+            CU_TRY(ctx, cudaEventElapsedTime(&t, ev[k], ev[k + 1]));
+            acc[k] += t;
+        }
+    }
+    for (int k = 0; k < 3; ++k) ms[k] = (float)(acc[k] / cnt);
+    *n_calls = cnt;
     return AFQMC_OK;
 }
 
