@@ -25,6 +25,8 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *   - Return value: AFQMC_OK or a negative error code; afqmc_last_error() gives the text.  Argument errors are
  *     detected before any work is enqueued.
+ *   - Tuning override (benchmarks only; results do not depend on it): the environment variable
+ *     AFQMC_K2_PIPELINE="k,s" forces K2's shared-memory ring to s stages of k DMMA k-steps each when that fits.
  *   - Requires compute capability 10.x (sm_100a); anything else returns AFQMC_ERR_ARCH.  There is no CPU path.
  */
 #ifndef AFQMC_H_
@@ -118,6 +120,11 @@ typedef struct afqmc_info {
 } afqmc_info;
 
 int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info);
+
+/* afqmc_plan -- host only (no CUDA call, works without a GPU): the K2 tile shape, pipeline depth and packed
+ * operand sizes afqmc_create would choose for these sizes (kernel_launches = 0).  Same argument checks and
+ * error codes as afqmc_create. */
+int afqmc_plan(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, afqmc_info *info);
 
 /* Per-kernel device times of energy calls.  enable != 0 makes every later afqmc_local_energy record CUDA
  * events around K1, K2 (both spins) and K3 on the caller's stream. */

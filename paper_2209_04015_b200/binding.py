@@ -15,7 +15,7 @@ _LIB = None
 
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
-           "afqmc_fp64_peak"]
+           "afqmc_fp64_peak", "afqmc_plan"]
 
 
 class AfqmcError(RuntimeError):
@@ -67,6 +67,8 @@ def load_library():
     lib.afqmc_mean_kernel_ms.restype = ip
     lib.afqmc_fp64_peak.argtypes = [ip, ip, C.POINTER(dp), vp]
     lib.afqmc_fp64_peak.restype = ip
+    lib.afqmc_plan.argtypes = [ip, ip, ip, ip, ip, C.POINTER(AfqmcInfo)]
+    lib.afqmc_plan.restype = ip
     _LIB = lib
     return lib
 
@@ -90,6 +92,24 @@ def fp64_peak_tflops(mode: str = "dmma", launches: int = 10) -> float:
     if rc != 0:
         raise AfqmcError(f"afqmc_fp64_peak failed ({rc}): {lib.afqmc_last_error(None).decode()}")
     return out.value
+
+
+def _info_dict(inf) -> dict:
+    out = {}
+    for name, _ in AfqmcInfo._fields_:
+        v = getattr(inf, name)
+        out[name] = list(v) if hasattr(v, "__len__") else v
+    return out
+
+
+def plan(N, n_alpha, n_beta, n_gamma, max_walkers) -> dict:
+    """afqmc_plan: the K2 tile shape / pipeline / packed sizes afqmc_create would choose (host only, no GPU)."""
+    lib = load_library()
+    inf = AfqmcInfo()
+    rc = lib.afqmc_plan(N, n_alpha, n_beta, n_gamma, max_walkers, C.byref(inf))
+    if rc != 0:
+        raise AfqmcError(f"afqmc_plan failed ({rc}): {lib.afqmc_last_error(None).decode()}")
+    return _info_dict(inf)
 
 
 class LocalEnergy:
@@ -159,11 +179,7 @@ class LocalEnergy:
     def info(self) -> dict:
         inf = AfqmcInfo()
         self._check(self._lib.afqmc_get_info(self._h, C.byref(inf)), "afqmc_get_info")
-        out = {}
-        for name, _ in AfqmcInfo._fields_:
-            v = getattr(inf, name)
-            out[name] = list(v) if hasattr(v, "__len__") else v
-        return out
+        return _info_dict(inf)
 
     def set_profiling(self, enable: bool):
         self._check(self._lib.afqmc_set_profiling(self._h, int(bool(enable))), "afqmc_set_profiling")

@@ -3,9 +3,11 @@
 // Every arithmetic step of the path runs in the kernels K0..K3 included below.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -75,10 +77,34 @@ int fail(afqmc_ctx *ctx, int code, const char *fmt, ...) {
                         cudaGetErrorString(e_));                                                            \
     } while (0)
 
-size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages, int LD) {
-    size_t stage = (size_t)ksc * (strips + NT) * 256;
-    return nstages * stage + (size_t)strips * 8 * LD * 8 + (size_t)8 * NT * 4 + (size_t)K2_MAX_WT * K2_MAX_WM * 16 +
-           (size_t)2 * nstages * 8 + 16;
+size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages, int LD, int n) {
+    const size_t stage = (size_t)ksc * (strips + NT) * 256;
+    return nstages * stage + (size_t)strips * 8 * LD * 8 + (size_t)(n * (n + 1) / 2) * 8 +
+           (size_t)K2_MAX_WT * K2_MAX_WM * 16 + (size_t)2 * nstages * 8 + 16;
+}
+
+// Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer,
+// preferring the most k-steps in flight (capped at 12), then the larger chunk.
+bool choose_pipeline(int strips, int NT, int LD, int n, int ksteps, int &ksc, int &nst) {
+    if (const char *ov = std::getenv("AFQMC_K2_PIPELINE")) {   // tuning override "ksc,stages" (include/afqmc.h)
+        int kc = 0, s = 0;
+        if (std::sscanf(ov, "%d,%d", &kc, &s) == 2 && kc >= 1 && kc <= ksteps && s >= 3 && s <= 16 &&
+            k2_smem_bytes(strips, NT, kc, s, LD, n) <= (size_t)kMaxSmem) {
+            ksc = kc; nst = s;
+            return true;
+        }
+    }
+    int best = 0;
+    for (int kc = 4; kc >= 1; --kc) {
+        if (kc > ksteps) continue;
+        for (int s = 8; s >= 3; --s) {
+            if (k2_smem_bytes(strips, NT, kc, s, LD, n) > (size_t)kMaxSmem) continue;
+            const int inflight = std::min(kc * s, 12);
+            if (inflight > best) { best = inflight; ksc = kc; nst = s; }
+            break;
+        }
+    }
+    return best > 0;
 }
 
 // Pick the K2 tile shape for one spin: maximise (useful rows / issued rows) x (useful cols / issued cols),
@@ -104,16 +130,9 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
                     if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
                     const int maxload = (strips + 3) / 4;
                     const double rowEff = (gT * n / 8.0) / (4.0 * maxload);
-                    const int LD = (2 * n) | 1;
-                    int ksc = 4, nst = 0;
-                    for (int s = 6; s >= 3; --s)
-                        if (k2_smem_bytes(strips, NT, ksc, s, LD) <= (size_t)kMaxSmem) { nst = s; break; }
-                    if (nst == 0) {
-                        ksc = 2;
-                        for (int s = 6; s >= 3; --s)
-                            if (k2_smem_bytes(strips, NT, ksc, s, LD) <= (size_t)kMaxSmem) { nst = s; break; }
-                    }
-                    if (nst == 0) continue;
+                    const int LD = 8 * NT + 1;
+                    int ksc = 0, nst = 0;
+                    if (!choose_pipeline(strips, NT, LD, n, ksteps, ksc, nst)) continue;
                     const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
                     const double fill = ntiles >= 148 ? 1.0 : ntiles / 148.0;
                     const double lds = 1.0 - 0.03 * (double)(MT + NT) / (MT * NT);
@@ -131,7 +150,7 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
     c.nchunks = (ksteps + c.ksc - 1) / c.ksc;
     c.n_rt = (n_gamma + c.gT - 1) / c.gT;
     c.n_ct_max = (maxw + c.wT - 1) / c.wT;
-    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages, c.LD);
+    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages, c.LD, n);
     c.layA = OperandLayout{n, c.strips, ksteps, c.gT, (long long)c.strips * ksteps * 32};
     c.layB = OperandLayout{n, c.NT, ksteps, c.wT, (long long)c.NT * ksteps * 32};
     c.A_bytes = (size_t)c.n_rt * c.layA.tile_doubles * 8;
@@ -380,20 +399,40 @@ void afqmc_destroy(afqmc_ctx *ctx) { free_ctx(ctx); }
 
 const char *afqmc_last_error(const afqmc_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
-int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info) {
-    if (!ctx || !info) return AFQMC_ERR_ARG;
+static void fill_info(afqmc_info *info, int N, int n_gamma, int maxw, const SpinCfg sp[2]) {
     std::memset(info, 0, sizeof *info);
-    info->N = ctx->N; info->n_alpha = ctx->sp[0].n; info->n_beta = ctx->sp[1].n; info->n_gamma = ctx->n_gamma;
-    info->max_walkers = ctx->maxw; info->k_steps = ctx->ksteps;
+    info->N = N; info->n_alpha = sp[0].n; info->n_beta = sp[1].n; info->n_gamma = n_gamma;
+    info->max_walkers = maxw; info->k_steps = (N + 3) / 4;
     for (int s = 0; s < 2; ++s) {
-        const SpinCfg &c = ctx->sp[s];
+        const SpinCfg &c = sp[s];
         info->tile_rows[s] = c.strips * 8; info->tile_cols[s] = c.NT * 8;
         info->gammas_per_tile[s] = c.gT; info->walkers_per_tile[s] = c.wT;
         info->warps_m[s] = c.WM; info->mt[s] = c.MT; info->nt[s] = c.NT; info->stages[s] = c.nstages;
         info->ksteps_per_chunk[s] = c.ksc; info->k2_smem_bytes[s] = (int)c.k2_smem;
         info->ltilde_bytes += (long long)c.A_bytes; info->theta_bytes += (long long)c.B_bytes;
     }
+}
+
+int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info) {
+    if (!ctx || !info) return AFQMC_ERR_ARG;
+    fill_info(info, ctx->N, ctx->n_gamma, ctx->maxw, ctx->sp);
     info->kernel_launches = ctx->launches;
+    return AFQMC_OK;
+}
+
+int afqmc_plan(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, afqmc_info *info) {
+    if (!info) return fail(nullptr, AFQMC_ERR_ARG, "afqmc_plan: null pointer argument");
+    if (N < 1 || n_gamma < 1 || max_walkers < 1 || n_alpha < 0 || n_beta < 0 || n_alpha > N || n_beta > N ||
+        n_alpha + n_beta < 1)
+        return fail(nullptr, AFQMC_ERR_ARG, "afqmc_plan: size out of range");
+    if (n_alpha > AFQMC_MAX_NOCC || n_beta > AFQMC_MAX_NOCC)
+        return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_plan: n_sigma > %d is not supported yet", AFQMC_MAX_NOCC);
+    SpinCfg sp[2];
+    const int ns[2] = {n_alpha, n_beta};
+    for (int s = 0; s < 2; ++s)
+        if (!choose_cfg(ns[s], N, n_gamma, max_walkers, sp[s]))
+            return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_plan: no K2 tile shape fits n_sigma=%d", ns[s]);
+    fill_info(info, N, n_gamma, max_walkers, sp);
     return AFQMC_OK;
 }
 
