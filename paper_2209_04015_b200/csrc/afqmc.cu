@@ -30,7 +30,7 @@ constexpr int kProfSets = 256;     // ring of per-call event quadruples kept whi
 
 struct SpinCfg {
     int n = 0;
-    int MT = 0, NT = 0, WM = 0, gT = 0, wT = 0, strips = 0, ksc = 0, nchunks = 0, nstages = 0, LD = 0;
+    int MT = 0, NT = 0, WM = 0, gT = 0, wT = 0, strips = 0, ksc = 0, nchunks = 0, nstages = 0, H = 0, LD2 = 0;
     int n_rt = 0, n_ct_max = 0;
     size_t k2_smem = 0, k1_smem = 0;
     OperandLayout layA{}, layB{};
@@ -77,19 +77,27 @@ int fail(afqmc_ctx *ctx, int code, const char *fmt, ...) {
                         cudaGetErrorString(e_));                                                            \
     } while (0)
 
-size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages, int LD, int n) {
+// Staging buffer of the K2 epilogue: rows stored in pairs, pitch LD2 = 1 (mod 16) doubles, odd row at +H, H = 8 (mod 16).
+void k2_staging_shape(int NT, int &H, int &LD2) {
+    H = 8 * NT + ((NT & 1) ? 0 : 8);
+    LD2 = H + 8 * NT;
+    while (LD2 % 16 != 1) ++LD2;
+}
+
+size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages) {
     const size_t stage = (size_t)ksc * (strips + NT) * 256;
-    return nstages * stage + (size_t)strips * 8 * LD * 8 + (size_t)(n * (n + 1) / 2) * 8 +
-           (size_t)K2_MAX_WT * K2_MAX_WM * 16 + (size_t)2 * nstages * 8 + 16;
+    int H = 0, LD2 = 0;
+    k2_staging_shape(NT, H, LD2);
+    return nstages * stage + (size_t)strips * 4 * LD2 * 8 + (size_t)K2_MAX_WT * K2_MAX_WM * 16 + (size_t)(2 * nstages + 2) * 8 + 16;
 }
 
 // Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer,
 // preferring the most k-steps in flight (capped at 12), then the larger chunk.
-bool choose_pipeline(int strips, int NT, int LD, int n, int ksteps, int &ksc, int &nst) {
+bool choose_pipeline(int strips, int NT, int ksteps, int &ksc, int &nst) {
     if (const char *ov = std::getenv("AFQMC_K2_PIPELINE")) {   // tuning override "ksc,stages" (include/afqmc.h)
         int kc = 0, s = 0;
         if (std::sscanf(ov, "%d,%d", &kc, &s) == 2 && kc >= 1 && kc <= ksteps && s >= 3 && s <= 16 &&
-            k2_smem_bytes(strips, NT, kc, s, LD, n) <= (size_t)kMaxSmem) {
+            k2_smem_bytes(strips, NT, kc, s) <= (size_t)kMaxSmem) {
             ksc = kc; nst = s;
             return true;
         }
@@ -98,7 +106,7 @@ bool choose_pipeline(int strips, int NT, int LD, int n, int ksteps, int &ksc, in
     for (int kc = 4; kc >= 1; --kc) {
         if (kc > ksteps) continue;
         for (int s = 8; s >= 3; --s) {
-            if (k2_smem_bytes(strips, NT, kc, s, LD, n) > (size_t)kMaxSmem) continue;
+            if (k2_smem_bytes(strips, NT, kc, s) > (size_t)kMaxSmem) continue;
             const int inflight = std::min(kc * s, 12);
             if (inflight > best) { best = inflight; ksc = kc; nst = s; }
             break;
@@ -130,9 +138,8 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
                     if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
                     const int maxload = (strips + 3) / 4;
                     const double rowEff = (gT * n / 8.0) / (4.0 * maxload);
-                    const int LD = 8 * NT + 1;
                     int ksc = 0, nst = 0;
-                    if (!choose_pipeline(strips, NT, LD, n, ksteps, ksc, nst)) continue;
+                    if (!choose_pipeline(strips, NT, ksteps, ksc, nst)) continue;
                     const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
                     const double fill = ntiles >= 148 ? 1.0 : ntiles / 148.0;
                     const double lds = 1.0 - 0.03 * (double)(MT + NT) / (MT * NT);
@@ -140,7 +147,7 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
                     if (score > best + 1e-12) {
                         best = score;
                         c.MT = MT; c.NT = NT; c.WM = WM; c.gT = gT; c.wT = wT; c.strips = strips;
-                        c.ksc = ksc; c.nstages = nst; c.LD = LD;
+                        c.ksc = ksc; c.nstages = nst;
                     }
                 }
             }
@@ -150,7 +157,8 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
     c.nchunks = (ksteps + c.ksc - 1) / c.ksc;
     c.n_rt = (n_gamma + c.gT - 1) / c.gT;
     c.n_ct_max = (maxw + c.wT - 1) / c.wT;
-    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages, c.LD, n);
+    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages);
+    k2_staging_shape(c.NT, c.H, c.LD2);
     c.layA = OperandLayout{n, c.strips, ksteps, c.gT, (long long)c.strips * ksteps * 32};
     c.layB = OperandLayout{n, c.NT, ksteps, c.wT, (long long)c.NT * ksteps * 32};
     c.A_bytes = (size_t)c.n_rt * c.layA.tile_doubles * 8;
@@ -268,7 +276,7 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         CR_TRY(cudaMalloc(&sc.A, sc.A_bytes));
         CR_TRY(cudaMalloc(&sc.B, sc.B_bytes));
         CR_TRY(cudaMalloc(&sc.tbuf, (size_t)max_walkers * n_gamma * 16));
-        CR_TRY(cudaMalloc(&sc.xpart, (size_t)sc.n_rt * max_walkers * 16));
+        CR_TRY(cudaMalloc(&sc.xpart, (size_t)sc.n_rt * k2_epilogue_warps(sc.WM) * max_walkers * 16));
         CR_TRY(cudaMemsetAsync(sc.A, 0, sc.A_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.B, 0, sc.B_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.tbuf, 0, (size_t)max_walkers * n_gamma * 16, stream));
@@ -338,7 +346,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
         p2.n = sc.n; p2.gT = sc.gT; p2.wT = sc.wT; p2.strips = sc.strips; p2.WM = sc.WM;
         p2.ksteps = ctx->ksteps; p2.ksc = sc.ksc; p2.nchunks = sc.nchunks; p2.nstages = sc.nstages;
         p2.n_rt = sc.n_rt; p2.n_ct = (n_walkers + sc.wT - 1) / sc.wT;
-        p2.n_gamma = ctx->n_gamma; p2.n_walkers = n_walkers; p2.maxw = ctx->maxw; p2.LD = sc.LD;
+        p2.n_gamma = ctx->n_gamma; p2.n_walkers = n_walkers; p2.maxw = ctx->maxw; p2.H = sc.H; p2.LD2 = sc.LD2;
         p2.tbuf = sc.tbuf; p2.xpart = sc.xpart;
         const long long ntiles = (long long)p2.n_rt * p2.n_ct;
         const int grid = (int)std::min<long long>(ntiles, ctx->num_sms);
@@ -353,7 +361,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     K3Params p3{};
     p3.n_gamma = ctx->n_gamma; p3.maxw = ctx->maxw; p3.e0 = ctx->e0;
     for (int s = 0; s < 2; ++s) {
-        p3.n[s] = ctx->sp[s].n; p3.n_rt[s] = ctx->sp[s].n_rt; p3.tbuf[s] = ctx->sp[s].tbuf; p3.xpart[s] = ctx->sp[s].xpart;
+        p3.n[s] = ctx->sp[s].n; p3.n_rt[s] = ctx->sp[s].n_rt * k2_epilogue_warps(ctx->sp[s].WM); p3.tbuf[s] = ctx->sp[s].tbuf; p3.xpart[s] = ctx->sp[s].xpart;
     }
     p3.e1 = ctx->e1; p3.logdet = ctx->logdet;
     p3.out_energy = reinterpret_cast<double *>(out_energies);

@@ -14,12 +14,16 @@
 // (strip s -> warp s % WM) times all NT 8-column blocks of the tile, i.e. up to MT*NT DMMA.8x8x4 accumulators,
 // complex arithmetic built from real tiles (real Ltilde x re/im planes of theta).
 #pragma once
+#include <type_traits>
 #include "common.cuh"
 
 namespace afqmc {
 
 constexpr int K2_MAX_WT = 4;       // walkers per CTA tile
 constexpr int K2_MAX_WM = 12;      // consumer warps
+
+// Number of epilogue warps for a CTA of WM warps: one per SM sub-partition, or every warp of a small CTA.
+__host__ __device__ inline int k2_epilogue_warps(int WM) { return WM >= 8 ? 4 : WM; }
 
 struct K2Params {
     const double *A;               // packed Ltilde of this spin
@@ -32,39 +36,130 @@ struct K2Params {
     int nstages;
     int n_rt, n_ct;                // row tiles (gamma), column tiles (walkers)
     int n_gamma, n_walkers, maxw;
-    int LD;                        // leading dimension (doubles) of the staging buffer: 8*NT + 1 (odd)
+    int H, LD2;                    // staging buffer: row pair pitch LD2 (= 1 mod 16), odd-row offset H (= 8 mod 16)
     double *tbuf;                  // [maxw][n_gamma][2]  traces of this spin
-    double *xpart;                 // [n_rt][maxw][2]     exchange partial sums of this spin
+    double *xpart;                 // [n_rt * NE][maxw][2]   exchange partial sums of this spin, one share per epilogue warp
 };
+
+// Shared-memory fragment load with a compile-time byte offset.  Loads and DMMAs are both `asm volatile`, so the
+// software pipeline below is emitted in exactly the order written.
+template <int OFF>
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+%2];\n" : "=d"(v) : "r"(addr), "n"(OFF));
+    return v;
+}
+
+// Ring position of the consumer side of the operand pipeline (identical in every warp).
+struct K2Ring {
+    uint32_t smem_base;            // shared-window address of stage 0
+    uint32_t stage_bytes, a_chunk_bytes, a_kstride;   // a_kstride = strips * 256
+    uint32_t full_bar, empty_bar;  // shared-window addresses of the barrier arrays
+    int nstages, ksc, nchunks, last_ks, ksteps;
+    int stage;
+    uint32_t phase;
+};
+
+__device__ __forceinline__ void mbar_wait_addr(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP_A:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra.uni WAIT_DONE_A;\n"
+        "bra.uni WAIT_LOOP_A;\n"
+        "WAIT_DONE_A:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+
+__device__ __forceinline__ bool mbar_test_addr(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+
+// Wait for a "full" barrier.  The producer warp keeps refilling released stages while it waits, so that the ring
+// cannot run dry behind warps that trail it (the epilogue warps).
+template <class Produce>
+__device__ __forceinline__ void k2_wait_full(uint32_t bar, uint32_t parity, const bool producer_warp, const int lane, Produce &produce_poll) {
+    if (producer_warp) {
+        while (!mbar_test_addr(bar, parity))
+            if (lane == 0) produce_poll();
+        __syncwarp();
+    } else {
+        mbar_wait_addr(bar, parity);
+    }
+}
+
+// One output tile of one warp: MM strips x NT column blocks, K loop over all chunks / k-steps of the tile.  Per k-step:
+// MM + NT fragment loads (256 contiguous bytes per warp each), then MM * NT DMMAs.  Loads and DMMAs are `asm volatile`
+// and the strip count MM is a template parameter, so the loop carries no predication and no reconvergence points.
+template <int MM, int NT, class Produce>
+__device__ __forceinline__ void k2_tile_mma(double (&acc)[MM][NT][2], K2Ring &R, const uint32_t frag_off, const uint32_t a_moff,
+                                            const bool producer_warp, Produce &produce_poll, const int lane) {
+#pragma unroll 1
+    for (int c = 0; c < R.nchunks; ++c) {
+        const int nks = (c == R.nchunks - 1) ? R.last_ks : R.ksc;
+        if (producer_warp) {                       // refill at most one released stage per chunk, never blocking
+            if (lane == 0) produce_poll();
+            __syncwarp();
+        }
+        k2_wait_full(R.full_bar + 8u * R.stage, R.phase, producer_warp, lane, produce_poll);
+        uint32_t pa = R.smem_base + R.stage * R.stage_bytes + frag_off;          // + warp * 256 + lane * 8 (in frag_off)
+        uint32_t pb = R.smem_base + R.stage * R.stage_bytes + R.a_chunk_bytes + 8u * lane;
+#pragma unroll 1
+        for (int ks = 0; ks < nks; ++ks) {
+            double a[MM], b[NT];
+#pragma unroll
+            for (int m = 0; m < MM; ++m) a[m] = lds_f64<0>(pa + m * a_moff);
+#pragma unroll
+            for (int q = 0; q < NT; ++q) b[q] = lds_f64<0>(pb + q * 256);
+#pragma unroll
+            for (int m = 0; m < MM; ++m)
+#pragma unroll
+                for (int q = 0; q < NT; ++q) dmma_m8n8k4(acc[m][q][0], acc[m][q][1], a[m], b[q]);
+            pa += R.a_kstride;
+            pb += NT * 256u;
+        }
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(R.empty_bar + 8u * R.stage) : "memory");
+        if (++R.stage == R.nstages) { R.stage = 0; R.phase ^= 1u; }
+    }
+}
 
 template <int MT, int NT>
 __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <= 32*K2_MAX_WM = 384: 384*168 <= 64K registers
     extern __shared__ __align__(128) unsigned char k2_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int WM = P.WM, n = P.n, LD = P.LD;
-    const int nthr_c = WM * 32;
+    const int WM = P.WM, n = P.n, H = P.H, LD2 = P.LD2;
+    const int NE = k2_epilogue_warps(WM);                // the last NE warps (the lightest) run the epilogue
+    const bool is_e = warp >= WM - NE;
+    const int e_idx = warp - (WM - NE);
 
     const uint32_t a_chunk_bytes = (uint32_t)P.ksc * P.strips * 256u;
     const uint32_t b_chunk_bytes = (uint32_t)P.ksc * NT * 256u;
     const uint32_t stage_bytes = a_chunk_bytes + b_chunk_bytes;
     unsigned char *stage_base = k2_smem;
-    double *staging = reinterpret_cast<double *>(k2_smem + (size_t)P.nstages * stage_bytes);   // [8*strips][LD]
-    const int npairs = n * (n + 1) / 2, upb = (npairs + 31) >> 5;                              // pairs i<=j; 32-pair units per block
-    int2 *pairtab = reinterpret_cast<int2 *>(staging + (size_t)P.strips * 8 * LD);             // [npairs] (i*LD+j, j*LD+i)
-    double *red = reinterpret_cast<double *>(pairtab + npairs);                                 // [K2_MAX_WT][K2_MAX_WM][2]
+    double *staging = reinterpret_cast<double *>(k2_smem + (size_t)P.nstages * stage_bytes);   // [4*strips][LD2]
+    double *red = staging + (size_t)P.strips * 4 * LD2;                                         // [K2_MAX_WT][K2_MAX_WM][2]
     uint64_t *full_bar = reinterpret_cast<uint64_t *>(red + K2_MAX_WT * K2_MAX_WM * 2);
     uint64_t *empty_bar = full_bar + P.nstages;
-
-    // pair table: k -> (i, j), i <= j, row-major over the upper triangle
-    for (int i = tid; i < n; i += blockDim.x) {
-        int k = i * n - (i * (i - 1)) / 2;
-        for (int j = i; j < n; ++j, ++k) pairtab[k] = make_int2(i * LD + j, j * LD + i);
-    }
+    uint64_t *stg_full = empty_bar + P.nstages;          // every warp has parked its accumulators of this tile
+    uint64_t *stg_free = stg_full + 1;                   // the epilogue warps are done reading the staging buffer
+    const int mma_warps = min(WM, P.strips);             // warps that own at least one strip
     if (tid == 0) {
         for (int s = 0; s < P.nstages; ++s) {
             mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], WM);
+            mbar_init(&empty_bar[s], mma_warps);
         }
+        mbar_init(stg_full, WM);
+        mbar_init(stg_free, NE);
         mbar_fence_init();
     }
     __syncthreads();
@@ -75,20 +170,20 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
     const int step_rt = (int)(gridDim.x / (unsigned)P.n_ct), step_ct = (int)(gridDim.x % (unsigned)P.n_ct);
     const int first_rt = (int)(blockIdx.x / (unsigned)P.n_ct), first_ct = (int)(blockIdx.x % (unsigned)P.n_ct);
 
-    // ---- producer: lane 0 of the LAST warp (the warp with the fewest strips, i.e. the most slack).  It runs
-    // `nstages - 2` chunks ahead of the consumers, so the stage it refills was released by every warp at least one
-    // chunk ago and its wait on the empty barrier does not stall.
-    const bool is_producer = (tid == (WM - 1) * 32);
+    // ---- producer: lane 0 of the last strip-owning warp (an epilogue warp, so it has slack).  It issues 1-D bulk async copies (TMA engine) of whole K-chunks of the packed
+    // operands into the ring.  It never blocks: once per k-step (and while it waits for its own data) it tests the
+    // empty barrier of the next stage to refill and issues the copies if every strip-owning warp has released it.
+    const bool producer_warp = (warp == mma_warps - 1);
     int p_rt = first_rt, p_ct = first_ct, p_chunk = 0, p_stage = 0;
     uint32_t p_phase = 0;
     const double *p_a = P.A + (long long)p_rt * P.tileA_doubles;
     const double *p_b = P.B + (long long)p_ct * P.tileB_doubles;
-    auto produce_one = [&]() {
+    auto produce_poll = [&]() {
         if (p_rt >= P.n_rt) return;
+        if (!mbar_test_addr(smem_u32(&empty_bar[p_stage]), p_phase ^ 1u)) return;
         const bool last = (p_chunk == P.nchunks - 1);
         const uint32_t ab = last ? (uint32_t)last_ks * P.strips * 256u : a_chunk_bytes;
         const uint32_t bb = last ? (uint32_t)last_ks * NT * 256u : b_chunk_bytes;
-        mbar_wait(&empty_bar[p_stage], p_phase ^ 1u);
         mbar_arrive_expect_tx(&full_bar[p_stage], ab + bb);
         unsigned char *dst = stage_base + (size_t)p_stage * stage_bytes;
         bulk_g2s(dst, p_a, ab, &full_bar[p_stage]);
@@ -105,112 +200,123 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
             ++p_chunk;
         }
     };
-    if (is_producer)
-        for (int d = 0; d < P.nstages - 2; ++d) produce_one();
+    if (producer_warp && lane == 0)
+        for (int d = 0; d < P.nstages; ++d) produce_poll();     // fresh barriers: fills the whole ring
 
-    // ---- consumers: all WM warps ----
+    // ---- every warp: strips warp, warp + WM, ... (my_mt of them: MT or MT - 1, uniform per warp) ----
     int my_mt = 0;
 #pragma unroll
     for (int m = 0; m < MT; ++m)
         if (warp + m * WM < P.strips) my_mt = m + 1;
 
-    int stage = 0;
-    uint32_t phase = 0;
-    for (int rt = first_rt, ct = first_ct; rt < P.n_rt;) {
-        double acc[MT][NT][2];
-#pragma unroll
-        for (int m = 0; m < MT; ++m)
-#pragma unroll
-            for (int q = 0; q < NT; ++q) { acc[m][q][0] = 0.0; acc[m][q][1] = 0.0; }
+    K2Ring R;
+    R.smem_base = smem_u32(stage_base); R.stage_bytes = stage_bytes; R.a_chunk_bytes = a_chunk_bytes;
+    R.a_kstride = (uint32_t)P.strips * 256u;
+    R.full_bar = smem_u32(full_bar); R.empty_bar = smem_u32(empty_bar);
+    R.nstages = P.nstages; R.ksc = P.ksc; R.nchunks = P.nchunks; R.last_ks = last_ks; R.ksteps = P.ksteps;
+    R.stage = 0; R.phase = 0;
+    const uint32_t frag_off = (uint32_t)warp * 256u + 8u * lane, a_moff = (uint32_t)WM * 256u;
 
-        for (int c = 0; c < P.nchunks; ++c) {
-            const int nks = (c == P.nchunks - 1) ? last_ks : P.ksc;
-            if (is_producer) produce_one();
+    // The tile loop is instantiated for the two possible strip counts so that the K loop carries no predication.
+    auto run_tiles = [&](auto mm_tag) {
+        constexpr int MM = decltype(mm_tag)::value;
+        constexpr int MMA = MM > 0 ? MM : 1;
+        uint32_t tpar = 0;                                      // parity of this CTA's tile counter
+        for (int rt = first_rt, ct = first_ct; rt < P.n_rt;) {
+            double acc[MMA][NT][2];
+            if constexpr (MM > 0) {
+#pragma unroll
+                for (int m = 0; m < MM; ++m)
+#pragma unroll
+                    for (int q = 0; q < NT; ++q) { acc[m][q][0] = 0.0; acc[m][q][1] = 0.0; }
+                k2_tile_mma<MM, NT>(acc, R, frag_off, a_moff, producer_warp, produce_poll, lane);
+            }
+
+            // ------------------------------ epilogue ------------------------------
+            // Phase 1 (all warps): park the accumulators in the whole-tile staging buffer with the tile's own
+            // row/column numbering (row = g*n + i, col = (plane*wT + wl)*n + j).  Rows are stored in pairs:
+            //     element (row, col)  ->  (row >> 1) * LD2 + (row & 1) * H + col,     H = 8 mod 16,  LD2 = 1 mod 16,
+            // which makes the fragment-order stores here, the row loads and the column loads of phase 2 all
+            // bank-conflict free (column loads 2-way when g*n is odd).  Then every warp except the epilogue warps
+            // goes straight on to the next tile.
+            mbar_wait(stg_free, tpar ^ 1u);                                    // previous tile has been read out
+            if constexpr (MM > 0) {
+#pragma unroll
+                for (int m = 0; m < MM; ++m) {
+                    const int row = (warp + m * WM) * 8 + (lane >> 2);
+                    double *dst = staging + (row >> 1) * LD2 + (row & 1) * H + 2 * (lane & 3);
+#pragma unroll
+                    for (int q = 0; q < NT; ++q) { dst[q * 8] = acc[m][q][0]; dst[q * 8 + 1] = acc[m][q][1]; }
+                }
+            }
             __syncwarp();
-            mbar_wait(&full_bar[stage], phase);
-            const double *As = reinterpret_cast<const double *>(stage_base + (size_t)stage * stage_bytes);
-            const double *Bs = reinterpret_cast<const double *>(stage_base + (size_t)stage * stage_bytes + a_chunk_bytes);
-            for (int ks = 0; ks < nks; ++ks) {
-                double a[MT], b[NT];
-#pragma unroll
-                for (int m = 0; m < MT; ++m)
-                    a[m] = (m < my_mt) ? As[(ks * P.strips + warp + m * WM) * 32 + lane] : 0.0;
-#pragma unroll
-                for (int q = 0; q < NT; ++q) b[q] = Bs[(ks * NT + q) * 32 + lane];
-#pragma unroll
-                for (int m = 0; m < MT; ++m) {
-                    if (m < my_mt) {
-#pragma unroll
-                        for (int q = 0; q < NT; ++q) dmma_m8n8k4(acc[m][q][0], acc[m][q][1], a[m], b[q]);
+            if (lane == 0) mbar_arrive(stg_full);
+            if (is_e) {
+                // Phase 2 (epilogue warps, which carry the fewest strips and so have the slack): one (gamma g, walker wl)
+                // block T = R + iI (n x n) per pass, lanes over j, loop over i:
+                //     Re x += R_ij R_ji - I_ij I_ji,    Im x += 2 R_ij I_ji   (sum_ij I_ij R_ji = sum_ij R_ij I_ji by relabelling),
+                //     t = sum_j T_jj.
+                // When the tile has fewer blocks than epilogue warps, each block's i range is split into `rs` parts.
+                const int g0 = rt * P.gT;
+                const int gvalid = min(P.gT, P.n_gamma - g0);
+                const int w0 = ct * P.wT;
+                const int wvalid = min(P.wT, P.n_walkers - w0);
+                const int planeoff = P.wT * n;
+                const int nblk = gvalid * wvalid;
+                const int rs = max(1, NE / nblk);
+                if (lane < K2_MAX_WT) { red[(lane * K2_MAX_WM + e_idx) * 2] = 0.0; red[(lane * K2_MAX_WM + e_idx) * 2 + 1] = 0.0; }
+                mbar_wait(stg_full, tpar);
+                for (int u = e_idx; u < nblk * rs; u += NE) {
+                    const int blk = u / rs, part = u - blk * rs;
+                    const int g = blk / wvalid, wl = blk - g * wvalid;
+                    const int i_lo = (part * n) / rs, i_hi = ((part + 1) * n) / rs;
+                    const int gn = g * n, cb = wl * n;
+                    double xr = 0.0, xi = 0.0, tr = 0.0, ti = 0.0;
+                    for (int j0 = 0; j0 < n; j0 += 32) {
+                        const int j = j0 + lane;
+                        if (j < n) {
+                            const int rj = gn + j;
+                            const double *colp = staging + (rj >> 1) * LD2 + (rj & 1) * H + cb;    // T[j][i] = colp[i]
+                            const double *rowp = staging + cb + j;                                  // T[i][j] = rowp[off(gn + i)]
+                            if (part == 0) { tr += colp[j]; ti += colp[planeoff + j]; }
+#pragma unroll 2
+                            for (int i = i_lo; i < i_hi; ++i) {
+                                const int ri = gn + i;
+                                const double *rp = rowp + (ri >> 1) * LD2 + (ri & 1) * H;
+                                const double a_r = rp[0], a_i = rp[planeoff];
+                                const double b_r = colp[i], b_i = colp[planeoff + i];
+                                xr = fma(a_r, b_r, xr);
+                                xr = fma(-a_i, b_i, xr);
+                                xi = fma(a_r, b_i, xi);
+                            }
+                        }
                     }
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty_bar[stage]);
-            if (++stage == P.nstages) { stage = 0; phase ^= 1u; }
-        }
-
-        // ------------------------------ epilogue ------------------------------
-        // Phase 1: every warp parks its accumulators in the whole-tile staging buffer, staging[row][col] with the
-        // tile's own row/column numbering (row = g*n + i, col = (plane*wT + wl)*n + j), leading dimension LD odd.
-        const int g0 = rt * P.gT;
-        const int gvalid = min(P.gT, P.n_gamma - g0);
-        const int w0 = ct * P.wT;
-        const int wvalid = min(P.wT, P.n_walkers - w0);
-        // (the previous tile's readers all passed its closing barrier, so the buffer is free)
-#pragma unroll
-        for (int m = 0; m < MT; ++m) {
-            if (m < my_mt) {
-                double *dst = staging + ((warp + m * WM) * 8 + (lane >> 2)) * LD + 2 * (lane & 3);
-#pragma unroll
-                for (int q = 0; q < NT; ++q) { dst[q * 8] = acc[m][q][0]; dst[q * 8 + 1] = acc[m][q][1]; }
-            }
-        }
-        named_bar_sync(1, nthr_c);                                         // staging full
-        // Phase 2: for every (walker wl, gamma g) block, x += sum_ij T_ij T_ji over the pair table (i <= j, weight 2
-        // off the diagonal) and t = sum_i T_ii.  Work unit = 32 consecutive pairs of one block; units are dealt to warps.
-        const int planeoff = P.wT * n;
-        for (int wl = 0; wl < wvalid; ++wl) {
-            double xr = 0.0, xi = 0.0;
-            for (int u = warp; u < gvalid * upb; u += WM) {
-                const int g = u / upb, kc = u - g * upb;
-                const double *Tre = staging + (g * n) * LD + wl * n;
-                const double *Tim = Tre + planeoff;
-                const int k = kc * 32 + lane;
-                if (k < npairs) {
-                    const int2 dm = pairtab[k];
-                    const double ar = Tre[dm.x], ai = Tim[dm.x], br = Tre[dm.y], bi = Tim[dm.y];
-                    const double wgt = (dm.x == dm.y) ? 1.0 : 2.0;
-                    double pr = ar * br; pr = fma(-ai, bi, pr);
-                    double pi = ar * bi; pi = fma(ai, br, pi);
-                    xr = fma(wgt, pr, xr);
-                    xi = fma(wgt, pi, xi);
-                }
-                if (kc == 0) {                                             // uniform per warp: trace of this block
-                    double tr = 0.0, ti = 0.0;
-                    for (int i = lane; i < n; i += 32) { tr += Tre[i * LD + i]; ti += Tim[i * LD + i]; }
-                    tr = warp_sum(tr);
-                    ti = warp_sum(ti);
+                    xr = warp_sum(xr); xi = warp_sum(xi);
+                    if (part == 0) { tr = warp_sum(tr); ti = warp_sum(ti); }
                     if (lane == 0) {
-                        double *tp = P.tbuf + ((long long)(w0 + wl) * P.n_gamma + g0 + g) * 2;
-                        tp[0] = tr; tp[1] = ti;
+                        if (part == 0) {
+                            double *tp = P.tbuf + ((long long)(w0 + wl) * P.n_gamma + g0 + g) * 2;
+                            tp[0] = tr; tp[1] = ti;
+                        }
+                        red[(wl * K2_MAX_WM + e_idx) * 2] += xr;
+                        red[(wl * K2_MAX_WM + e_idx) * 2 + 1] += 2.0 * xi;
                     }
                 }
+                __syncwarp();
+                if (lane < wvalid) {                     // this warp's share of x for the tile's walkers; K3 adds the shares
+                    double *xp = P.xpart + ((long long)(rt * NE + e_idx) * P.maxw + w0 + lane) * 2;
+                    xp[0] = red[(lane * K2_MAX_WM + e_idx) * 2]; xp[1] = red[(lane * K2_MAX_WM + e_idx) * 2 + 1];
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(stg_free);
             }
-            xr = warp_sum(xr);
-            xi = warp_sum(xi);
-            if (lane == 0) { red[(wl * K2_MAX_WM + warp) * 2] = xr; red[(wl * K2_MAX_WM + warp) * 2 + 1] = xi; }
+            tpar ^= 1u;
+            rt += step_rt; ct += step_ct;
+            if (ct >= P.n_ct) { ct -= P.n_ct; ++rt; }
         }
-        named_bar_sync(2, nthr_c);                                         // red[] complete
-        if (tid < wvalid) {
-            double sr = 0.0, si = 0.0;
-            for (int q = 0; q < WM; ++q) { sr += red[(tid * K2_MAX_WM + q) * 2]; si += red[(tid * K2_MAX_WM + q) * 2 + 1]; }
-            double *xp = P.xpart + ((long long)rt * P.maxw + w0 + tid) * 2;
-            xp[0] = sr; xp[1] = si;
-        }
-        rt += step_rt; ct += step_ct;
-        if (ct >= P.n_ct) { ct -= P.n_ct; ++rt; }
-    }
+    };
+    if (my_mt == MT) run_tiles(std::integral_constant<int, MT>{});
+    else run_tiles(std::integral_constant<int, MT - 1>{});
 }
 
 }  // namespace afqmc
