@@ -88,7 +88,7 @@ size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages) {
     const size_t stage = (size_t)ksc * (strips + NT) * 256;
     int H = 0, LD2 = 0;
     k2_staging_shape(NT, H, LD2);
-    return nstages * stage + (size_t)strips * 4 * LD2 * 8 + (size_t)K2_MAX_WT * K2_MAX_WM * 16 + (size_t)(2 * nstages + 2) * 8 + 16;
+    return nstages * stage + (size_t)strips * 4 * LD2 * 8 + (size_t)2 * K2_MAX_WT * K2_MAX_WM * 16 + (size_t)(2 * nstages + 2) * 8 + 16;
 }
 
 // Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer,
@@ -276,7 +276,7 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         CR_TRY(cudaMalloc(&sc.A, sc.A_bytes));
         CR_TRY(cudaMalloc(&sc.B, sc.B_bytes));
         CR_TRY(cudaMalloc(&sc.tbuf, (size_t)max_walkers * n_gamma * 16));
-        CR_TRY(cudaMalloc(&sc.xpart, (size_t)sc.n_rt * k2_epilogue_warps(sc.WM) * max_walkers * 16));
+        CR_TRY(cudaMalloc(&sc.xpart, (size_t)sc.n_rt * max_walkers * 16));
         CR_TRY(cudaMemsetAsync(sc.A, 0, sc.A_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.B, 0, sc.B_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.tbuf, 0, (size_t)max_walkers * n_gamma * 16, stream));
@@ -361,7 +361,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     K3Params p3{};
     p3.n_gamma = ctx->n_gamma; p3.maxw = ctx->maxw; p3.e0 = ctx->e0;
     for (int s = 0; s < 2; ++s) {
-        p3.n[s] = ctx->sp[s].n; p3.n_rt[s] = ctx->sp[s].n_rt * k2_epilogue_warps(ctx->sp[s].WM); p3.tbuf[s] = ctx->sp[s].tbuf; p3.xpart[s] = ctx->sp[s].xpart;
+        p3.n[s] = ctx->sp[s].n; p3.n_rt[s] = ctx->sp[s].n_rt; p3.tbuf[s] = ctx->sp[s].tbuf; p3.xpart[s] = ctx->sp[s].xpart;
     }
     p3.e1 = ctx->e1; p3.logdet = ctx->logdet;
     p3.out_energy = reinterpret_cast<double *>(out_energies);

@@ -22,9 +22,6 @@ namespace afqmc {
 constexpr int K2_MAX_WT = 4;       // walkers per CTA tile
 constexpr int K2_MAX_WM = 12;      // consumer warps
 
-// Number of epilogue warps for a CTA of WM warps: one per SM sub-partition, or every warp of a small CTA.
-__host__ __device__ inline int k2_epilogue_warps(int WM) { return WM >= 8 ? 4 : WM; }
-
 struct K2Params {
     const double *A;               // packed Ltilde of this spin
     const double *B;               // packed theta planes of this spin
@@ -38,7 +35,7 @@ struct K2Params {
     int n_gamma, n_walkers, maxw;
     int H, LD2;                    // staging buffer: row pair pitch LD2 (= 1 mod 16), odd-row offset H (= 8 mod 16)
     double *tbuf;                  // [maxw][n_gamma][2]  traces of this spin
-    double *xpart;                 // [n_rt * NE][maxw][2]   exchange partial sums of this spin, one share per epilogue warp
+    double *xpart;                 // [n_rt][maxw][2]     exchange partial sums of this spin
 };
 
 // Shared-memory fragment load with a compile-time byte offset.  Loads and DMMAs are both `asm volatile`, so the
@@ -138,20 +135,17 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
     extern __shared__ __align__(128) unsigned char k2_smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int WM = P.WM, n = P.n, H = P.H, LD2 = P.LD2;
-    const int NE = k2_epilogue_warps(WM);                // the last NE warps (the lightest) run the epilogue
-    const bool is_e = warp >= WM - NE;
-    const int e_idx = warp - (WM - NE);
 
     const uint32_t a_chunk_bytes = (uint32_t)P.ksc * P.strips * 256u;
     const uint32_t b_chunk_bytes = (uint32_t)P.ksc * NT * 256u;
     const uint32_t stage_bytes = a_chunk_bytes + b_chunk_bytes;
     unsigned char *stage_base = k2_smem;
     double *staging = reinterpret_cast<double *>(k2_smem + (size_t)P.nstages * stage_bytes);   // [4*strips][LD2]
-    double *red = staging + (size_t)P.strips * 4 * LD2;                                         // [K2_MAX_WT][K2_MAX_WM][2]
-    uint64_t *full_bar = reinterpret_cast<uint64_t *>(red + K2_MAX_WT * K2_MAX_WM * 2);
+    double *red = staging + (size_t)P.strips * 4 * LD2;                                         // [2][K2_MAX_WT][K2_MAX_WM][2]
+    uint64_t *full_bar = reinterpret_cast<uint64_t *>(red + 2 * K2_MAX_WT * K2_MAX_WM * 2);
     uint64_t *empty_bar = full_bar + P.nstages;
     uint64_t *stg_full = empty_bar + P.nstages;          // every warp has parked its accumulators of this tile
-    uint64_t *stg_free = stg_full + 1;                   // the epilogue warps are done reading the staging buffer
+    uint64_t *stg_free = stg_full + 1;                   // every warp is done reading the staging buffer
     const int mma_warps = min(WM, P.strips);             // warps that own at least one strip
     if (tid == 0) {
         for (int s = 0; s < P.nstages; ++s) {
@@ -159,7 +153,7 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
             mbar_init(&empty_bar[s], mma_warps);
         }
         mbar_init(stg_full, WM);
-        mbar_init(stg_free, NE);
+        mbar_init(stg_free, WM);
         mbar_fence_init();
     }
     __syncthreads();
@@ -237,8 +231,7 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
             // row/column numbering (row = g*n + i, col = (plane*wT + wl)*n + j).  Rows are stored in pairs:
             //     element (row, col)  ->  (row >> 1) * LD2 + (row & 1) * H + col,     H = 8 mod 16,  LD2 = 1 mod 16,
             // which makes the fragment-order stores here, the row loads and the column loads of phase 2 all
-            // bank-conflict free (column loads 2-way when g*n is odd).  Then every warp except the epilogue warps
-            // goes straight on to the next tile.
+            // bank-conflict free (column loads 2-way when g*n is odd).
             mbar_wait(stg_free, tpar ^ 1u);                                    // previous tile has been read out
             if constexpr (MM > 0) {
 #pragma unroll
@@ -251,27 +244,29 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(stg_full);
-            if (is_e) {
-                // Phase 2 (epilogue warps, which carry the fewest strips and so have the slack): one (gamma g, walker wl)
-                // block T = R + iI (n x n) per pass, lanes over j, loop over i:
+            {
+                // Phase 2 (all warps, once the whole tile is parked; the FP64 pipe is shared with the DMMAs, so these
+                // DFMAs are only cheap while no warp is feeding it DMMAs): one (gamma g, walker wl) block
+                // T = R + iI (n x n) per pass, lanes over j, loop over i:
                 //     Re x += R_ij R_ji - I_ij I_ji,    Im x += 2 R_ij I_ji   (sum_ij I_ij R_ji = sum_ij R_ij I_ji by relabelling),
                 //     t = sum_j T_jj.
-                // When the tile has fewer blocks than epilogue warps, each block's i range is split into `rs` parts.
+                // When the tile has fewer blocks than warps, each block's i range is split into `rs` parts.
                 const int g0 = rt * P.gT;
                 const int gvalid = min(P.gT, P.n_gamma - g0);
                 const int w0 = ct * P.wT;
                 const int wvalid = min(P.wT, P.n_walkers - w0);
                 const int planeoff = P.wT * n;
                 const int nblk = gvalid * wvalid;
-                const int rs = max(1, NE / nblk);
-                if (lane < K2_MAX_WT) { red[(lane * K2_MAX_WM + e_idx) * 2] = 0.0; red[(lane * K2_MAX_WM + e_idx) * 2 + 1] = 0.0; }
+                const int rs = max(1, WM / nblk);
+                double *redp = red + tpar * (K2_MAX_WT * K2_MAX_WM * 2);      // double-buffered by tile parity
+                if (lane < K2_MAX_WT) { redp[(lane * K2_MAX_WM + warp) * 2] = 0.0; redp[(lane * K2_MAX_WM + warp) * 2 + 1] = 0.0; }
                 mbar_wait(stg_full, tpar);
-                for (int u = e_idx; u < nblk * rs; u += NE) {
+                for (int u = warp; u < nblk * rs; u += WM) {
                     const int blk = u / rs, part = u - blk * rs;
                     const int g = blk / wvalid, wl = blk - g * wvalid;
                     const int i_lo = (part * n) / rs, i_hi = ((part + 1) * n) / rs;
                     const int gn = g * n, cb = wl * n;
-                    double xr = 0.0, xi = 0.0, tr = 0.0, ti = 0.0;
+                    double xr = 0.0, xi = 0.0, yr = 0.0, yi = 0.0, tr = 0.0, ti = 0.0;
                     for (int j0 = 0; j0 < n; j0 += 32) {
                         const int j = j0 + lane;
                         if (j < n) {
@@ -279,36 +274,49 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
                             const double *colp = staging + (rj >> 1) * LD2 + (rj & 1) * H + cb;    // T[j][i] = colp[i]
                             const double *rowp = staging + cb + j;                                  // T[i][j] = rowp[off(gn + i)]
                             if (part == 0) { tr += colp[j]; ti += colp[planeoff + j]; }
-#pragma unroll 2
-                            for (int i = i_lo; i < i_hi; ++i) {
-                                const int ri = gn + i;
-                                const double *rp = rowp + (ri >> 1) * LD2 + (ri & 1) * H;
-                                const double a_r = rp[0], a_i = rp[planeoff];
-                                const double b_r = colp[i], b_i = colp[planeoff + i];
+                            int i = i_lo;
+                            for (; i + 1 < i_hi; i += 2) {                                          // two independent chains
+                                const int r0 = gn + i, r1 = r0 + 1;
+                                const double *p0 = rowp + (r0 >> 1) * LD2 + (r0 & 1) * H;
+                                const double *p1 = rowp + (r1 >> 1) * LD2 + (r1 & 1) * H;
+                                const double a_r = p0[0], a_i = p0[planeoff], b_r = colp[i], b_i = colp[planeoff + i];
+                                const double c_r = p1[0], c_i = p1[planeoff], d_r = colp[i + 1], d_i = colp[planeoff + i + 1];
+                                xr = fma(a_r, b_r, xr); yr = fma(c_r, d_r, yr);
+                                xr = fma(-a_i, b_i, xr); yr = fma(-c_i, d_i, yr);
+                                xi = fma(a_r, b_i, xi); yi = fma(c_r, d_i, yi);
+                            }
+                            if (i < i_hi) {
+                                const int r0 = gn + i;
+                                const double *p0 = rowp + (r0 >> 1) * LD2 + (r0 & 1) * H;
+                                const double a_r = p0[0], a_i = p0[planeoff], b_r = colp[i], b_i = colp[planeoff + i];
                                 xr = fma(a_r, b_r, xr);
                                 xr = fma(-a_i, b_i, xr);
                                 xi = fma(a_r, b_i, xi);
                             }
                         }
                     }
-                    xr = warp_sum(xr); xi = warp_sum(xi);
+                    xr = warp_sum(xr + yr); xi = warp_sum(xi + yi);
                     if (part == 0) { tr = warp_sum(tr); ti = warp_sum(ti); }
                     if (lane == 0) {
                         if (part == 0) {
                             double *tp = P.tbuf + ((long long)(w0 + wl) * P.n_gamma + g0 + g) * 2;
                             tp[0] = tr; tp[1] = ti;
                         }
-                        red[(wl * K2_MAX_WM + e_idx) * 2] += xr;
-                        red[(wl * K2_MAX_WM + e_idx) * 2 + 1] += 2.0 * xi;
+                        redp[(wl * K2_MAX_WM + warp) * 2] += xr;
+                        redp[(wl * K2_MAX_WM + warp) * 2 + 1] += 2.0 * xi;
                     }
                 }
                 __syncwarp();
-                if (lane < wvalid) {                     // this warp's share of x for the tile's walkers; K3 adds the shares
-                    double *xp = P.xpart + ((long long)(rt * NE + e_idx) * P.maxw + w0 + lane) * 2;
-                    xp[0] = red[(lane * K2_MAX_WM + e_idx) * 2]; xp[1] = red[(lane * K2_MAX_WM + e_idx) * 2 + 1];
-                }
-                __syncwarp();
                 if (lane == 0) mbar_arrive(stg_free);
+                if (warp == WM - 1) {                    // the lightest warp adds the per-warp shares in a fixed order
+                    mbar_wait(stg_free, tpar);
+                    if (lane < wvalid) {
+                        double sr = 0.0, si = 0.0;
+                        for (int q = 0; q < WM; ++q) { sr += redp[(lane * K2_MAX_WM + q) * 2]; si += redp[(lane * K2_MAX_WM + q) * 2 + 1]; }
+                        double *xp = P.xpart + ((long long)rt * P.maxw + w0 + lane) * 2;
+                        xp[0] = sr; xp[1] = si;
+                    }
+                }
             }
             tpar ^= 1u;
             rt += step_rt; ct += step_ct;

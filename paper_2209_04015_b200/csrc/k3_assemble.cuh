@@ -12,9 +12,9 @@ constexpr int K3_THREADS = 128;
 struct K3Params {
     int n_gamma, maxw;
     int n[2];
-    int n_rt[2];              // number of x shares per walker: K2 row tiles x epilogue warps
+    int n_rt[2];
     const double *tbuf[2];    // [maxw][n_gamma][2]
-    const double *xpart[2];   // [n_rt][maxw][2]  (n_rt as above)
+    const double *xpart[2];   // [n_rt][maxw][2]
     const double *e1;         // [2][maxw][2]
     const double *logdet;     // [2][maxw][2]
     double e0;
