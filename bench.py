@@ -166,6 +166,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2209_04015_b200 import LocalEnergy, fp64_peak_tflops
+    from paper_2209_04015_b200.parallel import max_over_ranks as _max_over_ranks
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (this library has no CPU path)")
@@ -181,11 +182,7 @@ def main():
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world > 1:
-            t = torch.tensor([x], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            return float(t.item())
-        return x
+        return _max_over_ranks(x, device=dev)
 
     # ---- inputs: same Hamiltonian/trial on every rank, rank-specific walkers would come from the caller; here
     # every rank evaluates the config's Nw walkers (weak scaling: per-GPU work fixed).

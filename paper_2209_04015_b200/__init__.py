@@ -6,3 +6,4 @@ does not load the library; the first use does, and fails loudly if it has not be
 """
 from .binding import (AfqmcError, LocalEnergy, fp64_peak_tflops, library_path, load_library, plan)  # noqa: F401
 from .build import build_library  # noqa: F401
+from .parallel import gather_walker_results, max_over_ranks, walker_shard  # noqa: F401

@@ -6,13 +6,14 @@
 // tile passes once through shared memory for the transpose pairing T_ij T_ji, nothing of size Nw*Ngamma*n^2 is
 // ever written to global memory.
 //
-// Structure (B200): persistent CTAs, one per SM, WM warps.  Thread 0 doubles as the producer: it issues 1-D bulk
-// async copies (TMA engine) of contiguous K-chunks of the packed operands (common.cuh) into a ring of shared-memory
-// stages guarded by full/empty mbarriers, nstages-2 chunks ahead of the math (a 13th, dedicated producer warp would
-// round the CTA up to 16 warps of register allocation and cap the kernel at 128 registers per thread).
-// Every warp is a consumer: each owns up to MT 8-row strips
-// (strip s -> warp s % WM) times all NT 8-column blocks of the tile, i.e. up to MT*NT DMMA.8x8x4 accumulators,
-// complex arithmetic built from real tiles (real Ltilde x re/im planes of theta).
+// Structure (B200): persistent CTAs, one per SM, WM warps, every warp an MMA warp.  Each warp owns up to MT 8-row
+// strips (strip s -> warp s % WM, so the load is balanced over the 4 SM sub-partitions) times all NT 8-column blocks
+// of the tile, i.e. up to MT*NT DMMA.8x8x4 accumulators; complex arithmetic is built from real tiles (real Ltilde x
+// re/im planes of theta).  Lane 0 of the last strip-owning warp doubles as the producer: it issues 1-D
+// bulk async copies (TMA engine) of contiguous K-chunks of the packed operands (common.cuh) into a ring of
+// shared-memory stages guarded by full/empty mbarriers, and never blocks.  The epilogue hands the tile over through
+// two more mbarriers (staging full / staging free) instead of CTA-wide barriers.  DESIGN.md section 6 has the
+// measurements behind these choices.
 #pragma once
 #include <type_traits>
 #include "common.cuh"
