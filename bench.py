@@ -150,6 +150,9 @@ def main():
     ap.add_argument("--config", default="cu2o2", choices=["tiny", "small", "medium", "cu2o2", "large"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="also time the other four configs (device-resident, fewer steps) and add them as "
+                         "'other_configs' to the JSON line; generating 'large' takes a few minutes of host time")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -201,6 +204,7 @@ def main():
     outE_h = torch.empty(nw, dtype=torch.complex128).pin_memory()
     outO_h = torch.empty(nw, dtype=torch.complex128).pin_memory()
     info = le.info()
+    walkers_bytes = int(walkers.numel() * 16)
     stream = torch.cuda.current_stream()
 
     # ---- FP64 peak, measured live (roofline denominator) ------------------------------------------------
@@ -273,7 +277,12 @@ def main():
                 "algorithmic_flops_per_launch": flops_per_launch, "k2_ms_per_launch": k2_launch_ms,
                 "kernel_ms_per_step": {"k1": kms[0], "k2": kms[1], "k3": kms[2]}, "profiled_calls": kcalls,
                 "roofline_ms_per_step": t_roof_ms, "step_frac_of_roofline": t_roof_ms / (ms_total / args.steps),
-                "hbm_bytes_algorithmic_per_step": bytes_l}
+                "hbm_bytes_algorithmic_per_step": bytes_l,
+                # K1 (overlap / LU / inverse / theta): reads the walkers, writes the packed theta planes
+                "k1": {"algorithmic_bytes": int(walkers_bytes + info["theta_bytes"]),
+                       "achieved_gbs": (walkers_bytes + info["theta_bytes"]) / (kms[0] * 1e-3) * 1e-9,
+                       "hbm_peak_gbs": hbm_gbs,
+                       "note": "1 % of the step; bound by the latency of the shared-memory LU, not by HBM"}}
 
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N=1 only) ---------------------------------------
     cpu = None
@@ -288,6 +297,47 @@ def main():
                "sample": f"oracle rung O3 on walker 0, {'all' if frac == 1 else f'first 1/{frac} of the'} "
                          f"{inp.n_gamma} Cholesky vectors ({dt:.1f} s{', scaled by ' + str(frac) if frac > 1 else ''})"}
 
+    # ---- the other configs (north_star: report all five), device-resident timing only ------------------------
+    others = None
+    if args.all_configs and world == 1:
+        le.close()
+        del walkers, h1e, trial
+        torch.cuda.empty_cache()
+        others = {}
+        for name in ("tiny", "small", "medium", "cu2o2", "large"):
+            if name == args.config:
+                continue
+            oi = make_inputs(name)
+            ole = LocalEnergy(torch.from_numpy(oi.h1e).to(dev), torch.from_numpy(oi.chol).to(dev),
+                              torch.from_numpy(oi.trial_packed()).to(dev), oi.N, oi.n_alpha, oi.n_beta, oi.n_gamma,
+                              oi.e0, oi.n_walkers)
+            torch.cuda.empty_cache()
+            ow = torch.from_numpy(oi.walkers_packed()).to(dev)
+            oE = torch.empty(oi.n_walkers, dtype=torch.complex128, device=dev)
+            oO = torch.empty_like(oE)
+            nsteps = 3 if name == "large" else 20
+            for _ in range(3):
+                ole.local_energy(ow, oi.n_walkers, oE, oO)
+            torch.cuda.synchronize()
+            ole.set_profiling(True)
+            e0.record(stream)
+            for _ in range(nsteps):
+                ole.local_energy(ow, oi.n_walkers, oE, oO)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            oms = e0.elapsed_time(e1) / nsteps
+            okms, _ = ole.mean_kernel_ms()
+            ofl = 4.0 * oi.N * oi.n_gamma * oi.n_walkers * (oi.n_alpha ** 2 + oi.n_beta ** 2)
+            otf = ofl / (okms[1] * 1e-3) * 1e-12
+            oinfo = ole.info()
+            others[name] = {"walkers_per_s": oi.n_walkers / (oms * 1e-3), "ms_per_step": oms, "steps": nsteps,
+                            "k2_tflops": otf, "k2_frac_of_peak": otf / peak,
+                            "kernel_ms_per_step": {"k1": okms[0], "k2": okms[1], "k3": okms[2]},
+                            "k2_tile": {k: oinfo[k] for k in ("tile_rows", "tile_cols", "stages", "ksteps_per_chunk")}}
+            ole.close()
+            del ow, oE, oO, oi
+            torch.cuda.empty_cache()
+
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -295,7 +345,7 @@ def main():
                 "config": {**workload_desc(args.config, cfg, nw),
                            "parallelism": f"walker replicas x{world}, no data-path collective",
                            "l2": "no flush: per-step working set (packed Ltilde + theta + walkers = "
-                                 f"{(bytes_l + walkers.numel() * 16) / 1e6:.0f} MB) exceeds the 126 MB L2",
+                                 f"{(bytes_l + walkers_bytes) / 1e6:.0f} MB) exceeds the 126 MB L2",
                            "k2_tile": {k: info[k] for k in ("tile_rows", "tile_cols", "gammas_per_tile",
                                                             "walkers_per_tile", "warps_m", "mt", "nt", "stages",
                                                             "k2_smem_bytes")}},
@@ -306,6 +356,8 @@ def main():
                 "gpu_launches": int(gpu_launches),
                 "roofline": roofline,
                 "cpu_baseline": cpu}
+        if others is not None:
+            line["other_configs"] = others
         print(json.dumps(line), flush=True)
     le.close()
     if world > 1:

@@ -206,8 +206,10 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
 
     K2Ring R;
     R.smem_base = smem_u32(stage_base); R.stage_bytes = stage_bytes; R.a_chunk_bytes = a_chunk_bytes;
+    asm volatile("" : "+r"(R.smem_base));      // opaque: keeps the window address in a register (no S2R per chunk)
     R.a_kstride = (uint32_t)P.strips * 256u;
     R.full_bar = smem_u32(full_bar); R.empty_bar = smem_u32(empty_bar);
+    asm volatile("" : "+r"(R.full_bar), "+r"(R.empty_bar));
     R.nstages = P.nstages; R.ksc = P.ksc; R.nchunks = P.nchunks; R.last_ks = last_ks; R.ksteps = P.ksteps;
     R.stage = 0; R.phase = 0;
     const uint32_t frag_off = (uint32_t)warp * 256u + 8u * lane, a_moff = (uint32_t)WM * 256u;
