@@ -44,7 +44,7 @@ enum {
     AFQMC_ERR_ALLOC = -2,       /* cudaMalloc failed                                                    */
     AFQMC_ERR_CUDA = -3,        /* a CUDA call or kernel launch failed                                  */
     AFQMC_ERR_ARCH = -4,        /* device is not sm_100                                                 */
-    AFQMC_ERR_UNSUPPORTED = -5  /* valid input the library does not handle yet (complex trial, n > 64)  */
+    AFQMC_ERR_UNSUPPORTED = -5  /* valid input the library does not handle yet (n_sigma > 64)           */
 };
 
 #define AFQMC_MAX_NOCC 64 /* largest n_sigma supported (shared-memory LU and register-tile limits) */
@@ -55,8 +55,10 @@ enum {
  *   chol   device, float64 [n_gamma][N][N], Cholesky vectors L^gamma_pq, each slice symmetric (Eq. 3).
  *          Not retained: may be freed after the call returns.
  *   trial  device, complex128: alpha block [N][n_alpha] followed by beta block [N][n_beta] (columns =
- *          occupied orbitals; orthonormal columns expected).  The imaginary part must be
- *          identically zero (all of BASELINE.json's configs); a complex trial returns AFQMC_ERR_UNSUPPORTED.
+ *          occupied orbitals; orthonormal columns expected).  A spin block whose imaginary part is
+ *          identically zero (all of BASELINE.json's configs) takes the real-Ltilde path of PAPER.md:212 (two real
+ *          products per complex T); a block with a non-zero imaginary part takes the four-product path (Ltilde
+ *          stored as stacked Re / Im rows), at twice the arithmetic.  Non-finite entries return AFQMC_ERR_ARG.
  *   N >= 1; 0 <= n_alpha, n_beta <= min(N, AFQMC_MAX_NOCC); n_alpha + n_beta >= 1; n_gamma >= 1.
  *   e0     constant energy E0 added to every walker's energy.
  *   max_walkers >= 1 sizes the internal workspaces (theta, partial sums).

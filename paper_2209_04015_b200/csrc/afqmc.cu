@@ -35,6 +35,9 @@ struct SpinCfg {
     size_t k2_smem = 0, k1_smem = 0;
     OperandLayout layA{}, layB{};
     double *A = nullptr, *B = nullptr, *psi = nullptr, *ht = nullptr, *tbuf = nullptr, *xpart = nullptr;
+    double *psi_im = nullptr, *ht_im = nullptr;   // complex trial only
+    int nb = 0;                                   // rows of one gamma block of the A operand: n (real trial) or 2n
+    bool cplx = false;                            // this spin's trial block has a non-zero imaginary part
     size_t A_bytes = 0, B_bytes = 0;
 };
 
@@ -117,8 +120,10 @@ bool choose_pipeline(int strips, int NT, int ksteps, int &ksc, int &nst) {
 
 // Pick the K2 tile shape for one spin: maximise (useful rows / issued rows) x (useful cols / issued cols),
 // balanced over the 4 SM sub-partitions (strip s -> warp s % WM -> sub-partition s % 4).
-bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
+bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
     c.n = n;
+    const int nb = cplx ? 2 * n : n;      // rows per gamma block
+    c.nb = nb;
     if (n == 0) return true;
     const int ksteps = (N + 3) / 4;
     double best = -1.0;
@@ -133,11 +138,11 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
             for (int MT = 1; MT <= 4; ++MT) {
                 if (MT * NT > kMaxAcc) continue;
                 for (int gT = 1; gT <= n_gamma; ++gT) {
-                    const int strips = (gT * n + 7) / 8;
+                    const int strips = (gT * nb + 7) / 8;
                     if (strips > MT * WM) break;
                     if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
                     const int maxload = (strips + 3) / 4;
-                    const double rowEff = (gT * n / 8.0) / (4.0 * maxload);
+                    const double rowEff = (gT * nb / 8.0) / (4.0 * maxload);
                     int ksc = 0, nst = 0;
                     if (!choose_pipeline(strips, NT, ksteps, ksc, nst)) continue;
                     const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
@@ -163,7 +168,7 @@ bool choose_cfg(int n, int N, int n_gamma, int maxw, SpinCfg &c) {
     c.layB = OperandLayout{n, c.NT, ksteps, c.wT, (long long)c.NT * ksteps * 32};
     c.A_bytes = (size_t)c.n_rt * c.layA.tile_doubles * 8;
     c.B_bytes = (size_t)c.n_ct_max * c.layB.tile_doubles * 8;
-    c.k1_smem = (size_t)2 * n * n * 16 + (size_t)K1_PCHUNK * n * 16 + (size_t)K1_PCHUNK * n * 8 + (size_t)n * 4 + 16;
+    c.k1_smem = (size_t)2 * n * n * 16 + (size_t)K1_PCHUNK * n * 16 + (size_t)2 * K1_PCHUNK * n * 8 + (size_t)n * 4 + 16;
     return true;
 }
 
@@ -194,7 +199,7 @@ K2Fn k2_pick(int mt, int nt) {
 void free_ctx(afqmc_ctx *c) {
     if (!c) return;
     for (int s = 0; s < 2; ++s) {
-        cudaFree(c->sp[s].A); cudaFree(c->sp[s].B); cudaFree(c->sp[s].psi); cudaFree(c->sp[s].ht);
+        cudaFree(c->sp[s].A); cudaFree(c->sp[s].B); cudaFree(c->sp[s].psi); cudaFree(c->sp[s].ht); cudaFree(c->sp[s].psi_im); cudaFree(c->sp[s].ht_im);
         cudaFree(c->sp[s].tbuf); cudaFree(c->sp[s].xpart);
     }
     cudaFree(c->e1); cudaFree(c->logdet); cudaFree(c->h_walkers); cudaFree(c->h_outE); cudaFree(c->h_outO);
@@ -245,32 +250,41 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         }                                                                                                     \
     } while (0)
 
-    // trial: must be real ("a real-valued array rchol"); split into per-spin real [N][n] arrays
+    // trial: split into per-spin real planes [N][n].  A spin whose trial block is real ("a real-valued
+    // array rchol": all of BASELINE.json's configs) gets a real Ltilde and two real DMMA products per complex T; a
+    // complex block gets Ltilde = (Re, Im) stacked in every gamma block and four products.
     const size_t ntrial = (size_t)N * (n_alpha + n_beta);
     std::vector<double> trial_h(2 * ntrial);
     CR_TRY(cudaMemcpyAsync(trial_h.data(), trial, 2 * ntrial * sizeof(double), cudaMemcpyDeviceToHost, stream));
     CR_TRY(cudaStreamSynchronize(stream));
-    for (size_t k = 0; k < ntrial; ++k) {
-        if (trial_h[2 * k + 1] != 0.0 || !std::isfinite(trial_h[2 * k])) {
+    for (size_t k = 0; k < 2 * ntrial; ++k) {
+        if (!std::isfinite(trial_h[k])) {
             free_ctx(c);
-            return fail(nullptr, AFQMC_ERR_UNSUPPORTED,
-                        "afqmc_create: trial has a non-zero imaginary part (or a non-finite entry); complex trials are not supported yet");
+            return fail(nullptr, AFQMC_ERR_ARG, "afqmc_create: trial has a non-finite entry");
         }
     }
     size_t toff = 0;
     for (int s = 0; s < 2; ++s) {
         SpinCfg &sc = c->sp[s];
-        if (!choose_cfg(ns[s], N, n_gamma, max_walkers, sc)) {
-            free_ctx(c);
-            return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: no K2 tile shape fits n_sigma=%d", ns[s]);
-        }
         const int n = ns[s];
+        bool cplx = false;
+        for (size_t k = 0; k < (size_t)N * n; ++k) cplx = cplx || (trial_h[2 * (toff + k) + 1] != 0.0);
+        sc.cplx = cplx;
+        if (!choose_cfg(n, cplx, N, n_gamma, max_walkers, sc)) {
+            free_ctx(c);
+            return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: no K2 tile shape fits n_sigma=%d", n);
+        }
         if (n == 0) continue;
-        std::vector<double> psi_h((size_t)N * n);
-        for (size_t k = 0; k < psi_h.size(); ++k) psi_h[k] = trial_h[2 * (toff + k)];
+        std::vector<double> psi_h((size_t)N * n), psi_ih((size_t)N * n);
+        for (size_t k = 0; k < psi_h.size(); ++k) { psi_h[k] = trial_h[2 * (toff + k)]; psi_ih[k] = trial_h[2 * (toff + k) + 1]; }
         toff += (size_t)N * n;
         CR_TRY(cudaMalloc(&sc.psi, psi_h.size() * 8));
         CR_TRY(cudaMemcpyAsync(sc.psi, psi_h.data(), psi_h.size() * 8, cudaMemcpyHostToDevice, stream));
+        if (cplx) {
+            CR_TRY(cudaMalloc(&sc.psi_im, psi_ih.size() * 8));
+            CR_TRY(cudaMemcpyAsync(sc.psi_im, psi_ih.data(), psi_ih.size() * 8, cudaMemcpyHostToDevice, stream));
+            CR_TRY(cudaMalloc(&sc.ht_im, (size_t)n * N * 8));
+        }
         CR_TRY(cudaStreamSynchronize(stream));
         CR_TRY(cudaMalloc(&sc.ht, (size_t)n * N * 8));
         CR_TRY(cudaMalloc(&sc.A, sc.A_bytes));
@@ -280,12 +294,19 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         CR_TRY(cudaMemsetAsync(sc.A, 0, sc.A_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.B, 0, sc.B_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.tbuf, 0, (size_t)max_walkers * n_gamma * 16, stream));
-        k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi, N, n, sc.ht);
-        CR_TRY(cudaGetLastError());
         dim3 grid((N + 127) / 128, n_gamma);
-        k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, sc.layA, sc.A);
+        k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi, N, n, 1.0, sc.ht);
+        CR_TRY(cudaGetLastError());
+        k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, sc.nb, 0, 1.0, sc.layA, sc.A);
         CR_TRY(cudaGetLastError());
         c->launches += 2;
+        if (cplx) {                                   // conj(psi) = Re psi - i Im psi
+            k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi_im, N, n, -1.0, sc.ht_im);
+            CR_TRY(cudaGetLastError());
+            k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi_im, N, n, n_gamma, sc.nb, n, -1.0, sc.layA, sc.A);
+            CR_TRY(cudaGetLastError());
+            c->launches += 2;
+        }
         K2Fn fn = k2_pick(sc.MT, sc.NT);
         if (!fn) {
             free_ctx(c);
@@ -327,6 +348,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     p1.spin_off[1] = (long long)n_walkers * N * ctx->sp[0].n;
     for (int s = 0; s < 2; ++s) {
         p1.n[s] = ctx->sp[s].n; p1.psi[s] = ctx->sp[s].psi; p1.ht[s] = ctx->sp[s].ht;
+        p1.psi_im[s] = ctx->sp[s].psi_im; p1.ht_im[s] = ctx->sp[s].ht_im;
         p1.thetaB[s] = ctx->sp[s].B; p1.layB[s] = ctx->sp[s].layB;
     }
     p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
@@ -343,7 +365,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
         K2Params p2{};
         p2.A = sc.A; p2.B = sc.B;
         p2.tileA_doubles = sc.layA.tile_doubles; p2.tileB_doubles = sc.layB.tile_doubles;
-        p2.n = sc.n; p2.gT = sc.gT; p2.wT = sc.wT; p2.strips = sc.strips; p2.WM = sc.WM;
+        p2.n = sc.n; p2.nb = sc.nb; p2.cplx = sc.cplx ? 1 : 0; p2.gT = sc.gT; p2.wT = sc.wT; p2.strips = sc.strips; p2.WM = sc.WM;
         p2.ksteps = ctx->ksteps; p2.ksc = sc.ksc; p2.nchunks = sc.nchunks; p2.nstages = sc.nstages;
         p2.n_rt = sc.n_rt; p2.n_ct = (n_walkers + sc.wT - 1) / sc.wT;
         p2.n_gamma = ctx->n_gamma; p2.n_walkers = n_walkers; p2.maxw = ctx->maxw; p2.H = sc.H; p2.LD2 = sc.LD2;
@@ -438,7 +460,7 @@ int afqmc_plan(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, afq
     SpinCfg sp[2];
     const int ns[2] = {n_alpha, n_beta};
     for (int s = 0; s < 2; ++s)
-        if (!choose_cfg(ns[s], N, n_gamma, max_walkers, sp[s]))
+        if (!choose_cfg(ns[s], false, N, n_gamma, max_walkers, sp[s]))
             return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_plan: no K2 tile shape fits n_sigma=%d", ns[s]);
     fill_info(info, N, n_gamma, max_walkers, sp);
     return AFQMC_OK;

@@ -1,21 +1,23 @@
 // K0 -- one-time half-rotation (Eq. 21), executed by afqmc_create, not on the timed path.
-//   htilde_sigma[i][p]       = sum_q psi[q][i] h[q][p]
-//   Ltilde^gamma_sigma[i][r] = sum_p psi[p][i] L^gamma[p][r]      (real trial => real Ltilde)
-// Ltilde is written straight into K2's packed A-operand layout (common.cuh).
+//   htilde_sigma[i][p]       = sum_q conj(psi[q][i]) h[q][p]
+//   Ltilde^gamma_sigma[i][r] = sum_p conj(psi[p][i]) L^gamma[p][r]      (real trial => real Ltilde)
+// Ltilde is written straight into K2's packed A-operand layout (common.cuh).  Both kernels work on one real plane of
+// psi at a time (`scale` = +1 for Re psi, -1 for Im psi because of the conjugate); for a complex trial the imaginary
+// plane of Ltilde occupies rows n..2n-1 of every gamma block (`row_shift` = n, `rows_per_gamma` = 2n).
 #pragma once
 #include "common.cuh"
 
 namespace afqmc {
 
 // htilde: one thread per (i, p).
-__global__ void k0_half_rotate_h(const double *__restrict__ h1e, const double *__restrict__ psi,  // psi [N][n] real
-                                 int N, int n, double *__restrict__ ht /* [n][N] */) {
+__global__ void k0_half_rotate_h(const double *__restrict__ h1e, const double *__restrict__ psi,  // psi plane [N][n]
+                                 int N, int n, double scale, double *__restrict__ ht /* [n][N] */) {
     int idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= n * N) return;
     int i = idx / N, p = idx - i * N;
     double acc = 0.0;
     for (int q = 0; q < N; ++q) acc = fma(psi[(size_t)q * n + i], h1e[(size_t)q * N + p], acc);
-    ht[idx] = acc;
+    ht[idx] = scale * acc;
 }
 
 // Ltilde: grid = (ceil(N/128), n_gamma); thread owns one (gamma, r) and produces all i in blocks of 8.
@@ -24,13 +26,13 @@ constexpr int K0_PCHUNK = 64;
 
 __global__ void __launch_bounds__(128)
 k0_half_rotate_chol(const double *__restrict__ chol, const double *__restrict__ psi, int N, int n, int n_gamma,
-                    OperandLayout lay, double *__restrict__ packedA) {
+                    int rows_per_gamma, int row_shift, double scale, OperandLayout lay, double *__restrict__ packedA) {
     __shared__ double psi_s[K0_PCHUNK * 8];  // [K0_PCHUNK][8]
     const int g = blockIdx.y;
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     const double *Lg = chol + (size_t)g * N * N;
     const int tile = g / lay.per_tile;
-    const int row0 = (g - tile * lay.per_tile) * n;
+    const int row0 = (g - tile * lay.per_tile) * rows_per_gamma + row_shift;
     for (int i0 = 0; i0 < n; i0 += 8) {
         double acc[8];
 #pragma unroll
@@ -54,7 +56,7 @@ k0_half_rotate_chol(const double *__restrict__ chol, const double *__restrict__ 
         if (r < N) {
 #pragma unroll
             for (int k = 0; k < 8; ++k)
-                if (i0 + k < n) packedA[packed_offset(lay, tile, row0 + i0 + k, r)] = acc[k];
+                if (i0 + k < n) packedA[packed_offset(lay, tile, row0 + i0 + k, r)] = scale * acc[k];
         }
     }
 }

@@ -1,5 +1,5 @@
 // K1 -- per (walker, spin): overlap matrix, LU with partial pivoting, log-determinant, inverse, theta, E1.
-//   S      = psi^T phi                      (n x n; real trial)              PAPER.md:143 (Eq. 16), Listing 2 line 1
+//   S      = psi^dagger phi                 (n x n)                          PAPER.md:143 (Eq. 16), Listing 2 line 1
 //   P S    = L U, log det S                                                   PAPER.md:146-150 ("linalg.det"), Listing 2 line 2
 //   X      = S^-1
 //   theta  = (phi X)^T  (n x N), written as separate re / im planes           PAPER.md:191 (Eq. 23), Listing 2 line 3;
@@ -20,8 +20,10 @@ struct K1Params {
     int n_walkers, N, maxw;
     int n[2];
     long long spin_off[2];        // offset of each spin block in `walkers`, in complex elements
-    const double *psi[2];         // [N][n] real
-    const double *ht[2];          // [n][N] real
+    const double *psi[2];         // [N][n] Re psi
+    const double *ht[2];          // [n][N] Re htilde
+    const double *psi_im[2];      // Im psi, or nullptr for a real trial block
+    const double *ht_im[2];       // Im htilde, or nullptr
     double *thetaB[2];            // packed B operand
     OperandLayout layB[2];
     double *logdet;               // [2][maxw][2]  (log|det|, arg)
@@ -41,15 +43,18 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
     double2 *S = reinterpret_cast<double2 *>(k1_smem);        // [n][n]
     double2 *X = S + n * n;                                   // [n][n]
     double2 *phis = X + n * n;                                // [K1_PCHUNK][n]
-    double *psis = reinterpret_cast<double *>(phis + K1_PCHUNK * n);  // [K1_PCHUNK][n]
-    int *perm = reinterpret_cast<int *>(psis + K1_PCHUNK * n);        // [n]
+    double *psis = reinterpret_cast<double *>(phis + K1_PCHUNK * n);  // [K1_PCHUNK][n]  Re psi
+    double *psii = psis + K1_PCHUNK * n;                              // [K1_PCHUNK][n]  Im psi (complex trial)
+    int *perm = reinterpret_cast<int *>(psii + K1_PCHUNK * n);        // [n]
     __shared__ int s_piv;
     __shared__ double s_red[2 * (K1_THREADS / 32)];
 
     const double2 *phi = P.walkers + P.spin_off[sp] + (long long)w * N * n;   // [N][n]
     const double *psi = P.psi[sp];
+    const double *psi_im = P.psi_im[sp];
+    const bool cplx = psi_im != nullptr;
 
-    // ---- S = psi^T phi ------------------------------------------------------------------------
+    // ---- S = psi^dagger phi = (Re psi - i Im psi)^T phi ------------------------------------------------------------------------
     for (int e = tid; e < n * n; e += K1_THREADS) S[e] = make_double2(0.0, 0.0);
     for (int p0 = 0; p0 < N; p0 += K1_PCHUNK) {
         const int pc = min(K1_PCHUNK, N - p0);
@@ -57,6 +62,7 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
         for (int t = tid; t < pc * n; t += K1_THREADS) {
             phis[t] = phi[(long long)p0 * n + t];
             psis[t] = psi[(long long)p0 * n + t];
+            if (cplx) psii[t] = psi_im[(long long)p0 * n + t];
         }
         __syncthreads();
         for (int e = tid; e < n * n; e += K1_THREADS) {
@@ -67,6 +73,14 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
                 const double2 f = phis[pp * n + j];
                 acc.x = fma(a, f.x, acc.x);
                 acc.y = fma(a, f.y, acc.y);
+            }
+            if (cplx) {
+                for (int pp = 0; pp < pc; ++pp) {
+                    const double b = psii[pp * n + i];
+                    const double2 f = phis[pp * n + j];
+                    acc.x = fma(b, f.y, acc.x);        // (a - ib)(fx + i fy) = (a fx + b fy) + i (a fy - b fx)
+                    acc.y = fma(-b, f.x, acc.y);
+                }
             }
             S[e] = acc;
         }
@@ -181,6 +195,7 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
     const int col_re = wl * n, col_im = (wT + wl) * n;
     double *out = P.thetaB[sp];
     const double *ht = P.ht[sp];
+    const double *ht_im = P.ht_im[sp];
     const int kk = lane & 3, jj = lane >> 2;
     double e1r = 0.0, e1i = 0.0;
     const int Kpad = lay.ksteps * 4;
@@ -204,6 +219,11 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
                     const double hv = ht[(long long)j * N + p];
                     e1r = fma(hv, acc.x, e1r);
                     e1i = fma(hv, acc.y, e1i);
+                    if (cplx) {
+                        const double hi = ht_im[(long long)j * N + p];
+                        e1r = fma(-hi, acc.y, e1r);
+                        e1i = fma(hi, acc.x, e1i);
+                    }
                 }
                 out[packed_offset(lay, tile, col_re + j, p)] = acc.x;
                 out[packed_offset(lay, tile, col_im + j, p)] = acc.y;

@@ -28,6 +28,7 @@ struct K2Params {
     const double *B;               // packed theta planes of this spin
     long long tileA_doubles, tileB_doubles;
     int n, gT, wT;                 // electrons, gamma-blocks per tile, walkers per tile
+    int nb, cplx;                  // rows per gamma block of A: n (real Ltilde) or 2n (rows n..2n-1 = Im Ltilde, cplx = 1)
     int strips;                    // 8-row strips per A tile
     int WM;                        // consumer warps
     int ksteps, ksc, nchunks;      // total k-steps, k-steps per chunk, chunks per tile
@@ -231,7 +232,7 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
 
             // ------------------------------ epilogue ------------------------------
             // Phase 1 (all warps): park the accumulators in the whole-tile staging buffer with the tile's own
-            // row/column numbering (row = g*n + i, col = (plane*wT + wl)*n + j).  Rows are stored in pairs:
+            // row/column numbering (row = g*nb + i, col = (plane*wT + wl)*n + j).  Rows are stored in pairs:
             //     element (row, col)  ->  (row >> 1) * LD2 + (row & 1) * H + col,     H = 8 mod 16,  LD2 = 1 mod 16,
             // which makes the fragment-order stores here, the row loads and the column loads of phase 2 all
             // bank-conflict free (column loads 2-way when g*n is odd).
@@ -268,30 +269,38 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
                     const int blk = u / rs, part = u - blk * rs;
                     const int g = blk / wvalid, wl = blk - g * wvalid;
                     const int i_lo = (part * n) / rs, i_hi = ((part + 1) * n) / rs;
-                    const int gn = g * n, cb = wl * n;
+                    const int gn = g * P.nb, cb = wl * n;
+                    const bool cplx = P.cplx != 0;
+                    // element T_ij = R + iI of the block, from the parked products C = Ltilde theta^T:
+                    //   real Ltilde:     R = C[i][re j],                   I = C[i][im j]
+                    //   complex Ltilde:  R = C[re i][re j] - C[im i][im j], I = C[re i][im j] + C[im i][re j]   (rows im i = n + i)
+                    auto elem = [&](const double *p, int row, int col, double &re, double &im) {
+                        const double *q = p + (row >> 1) * LD2 + (row & 1) * H + col;
+                        re = q[0]; im = q[planeoff];
+                        if (cplx) {
+                            const int r2 = row + n;
+                            const double *q2 = p + (r2 >> 1) * LD2 + (r2 & 1) * H + col;
+                            re -= q2[planeoff]; im += q2[0];
+                        }
+                    };
                     double xr = 0.0, xi = 0.0, yr = 0.0, yi = 0.0, tr = 0.0, ti = 0.0;
                     for (int j0 = 0; j0 < n; j0 += 32) {
                         const int j = j0 + lane;
                         if (j < n) {
-                            const int rj = gn + j;
-                            const double *colp = staging + (rj >> 1) * LD2 + (rj & 1) * H + cb;    // T[j][i] = colp[i]
-                            const double *rowp = staging + cb + j;                                  // T[i][j] = rowp[off(gn + i)]
-                            if (part == 0) { tr += colp[j]; ti += colp[planeoff + j]; }
+                            const double *blkp = staging + cb;
+                            if (part == 0) { double r, im; elem(blkp, gn + j, j, r, im); tr += r; ti += im; }
                             int i = i_lo;
                             for (; i + 1 < i_hi; i += 2) {                                          // two independent chains
-                                const int r0 = gn + i, r1 = r0 + 1;
-                                const double *p0 = rowp + (r0 >> 1) * LD2 + (r0 & 1) * H;
-                                const double *p1 = rowp + (r1 >> 1) * LD2 + (r1 & 1) * H;
-                                const double a_r = p0[0], a_i = p0[planeoff], b_r = colp[i], b_i = colp[planeoff + i];
-                                const double c_r = p1[0], c_i = p1[planeoff], d_r = colp[i + 1], d_i = colp[planeoff + i + 1];
+                                double a_r, a_i, b_r, b_i, c_r, c_i, d_r, d_i;
+                                elem(blkp, gn + i, j, a_r, a_i); elem(blkp, gn + j, i, b_r, b_i);            // T_ij, T_ji
+                                elem(blkp, gn + i + 1, j, c_r, c_i); elem(blkp, gn + j, i + 1, d_r, d_i);
                                 xr = fma(a_r, b_r, xr); yr = fma(c_r, d_r, yr);
                                 xr = fma(-a_i, b_i, xr); yr = fma(-c_i, d_i, yr);
                                 xi = fma(a_r, b_i, xi); yi = fma(c_r, d_i, yi);
                             }
                             if (i < i_hi) {
-                                const int r0 = gn + i;
-                                const double *p0 = rowp + (r0 >> 1) * LD2 + (r0 & 1) * H;
-                                const double a_r = p0[0], a_i = p0[planeoff], b_r = colp[i], b_i = colp[planeoff + i];
+                                double a_r, a_i, b_r, b_i;
+                                elem(blkp, gn + i, j, a_r, a_i); elem(blkp, gn + j, i, b_r, b_i);
                                 xr = fma(a_r, b_r, xr);
                                 xr = fma(-a_i, b_i, xr);
                                 xi = fma(a_r, b_i, xi);

@@ -84,7 +84,7 @@ def test_parity_full_size_vs_golden(name):
 
 
 # ---- edge cases --------------------------------------------------------------------------------------
-def _custom(seed, N, na, nb, ng, nw, noise=0.2):
+def _custom(seed, N, na, nb, ng, nw, noise=0.2, complex_trial=False):
     rng = np.random.default_rng(seed)
     a = rng.standard_normal((N, N))
     h = 0.5 * (a + a.T) + np.diag(np.arange(N, dtype=float))
@@ -94,6 +94,12 @@ def _custom(seed, N, na, nb, ng, nw, noise=0.2):
     psi_a = q[:, :na].astype(np.complex128)
     q2, _ = np.linalg.qr(rng.standard_normal((N, N)))
     psi_b = q2[:, :nb].astype(np.complex128)
+    if complex_trial:        # orthonormal complex columns: Q factor of a complex Gaussian matrix
+        qa, _ = np.linalg.qr(rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N)))
+        psi_a = qa[:, :na]
+        if complex_trial == "both":
+            qb, _ = np.linalg.qr(rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N)))
+            psi_b = qb[:, :nb]
     phi_a = psi_a[None] + noise * (rng.standard_normal((nw, N, na)) + 1j * rng.standard_normal((nw, N, na)))
     phi_b = psi_b[None] + noise * (rng.standard_normal((nw, N, nb)) + 1j * rng.standard_normal((nw, N, nb)))
     return Inputs(name="custom", N=N, n_alpha=na, n_beta=nb, n_gamma=ng, e0=-1.25, h1e=h, chol=chol,
@@ -115,6 +121,30 @@ def test_parity_edge_shapes(N, na, nb, ng, nw):
     Eo, loo = orc.local_energy_batch(inp, rung="O1" if N <= 40 else "O3")
     E, lo = gpu_energy(inp)
     assert_parity(E, lo, Eo, loo)
+
+
+@pytest.mark.parametrize("N,na,nb,ng,nw,which", [
+    (12, 5, 2, 9, 3, "both"),      # complex trial in both spins (4-product path), odd sizes
+    (12, 4, 3, 9, 3, True),        # complex alpha block, real beta block
+    (33, 13, 11, 70, 7, "both"),   # several row tiles, ragged tails
+    (70, 33, 31, 41, 5, "both"),   # 2n = 66 rows per gamma block, n > 32 (two lane chunks)
+    (9, 3, 0, 7, 2, True),         # no beta electrons
+])
+def test_parity_complex_trial(N, na, nb, ng, nw, which):
+    """Complex (non-real) trial: Ltilde is complex and T needs four real products (Eq. 21
+    with a complex psi).  The oracle is the same definition (it never forms Ltilde)."""
+    inp = _custom(300 + N, N, na, nb, ng, nw, complex_trial=which)
+    Eo, loo = orc.local_energy_batch(inp, rung="O1" if N <= 40 else "O3")
+    E, lo = gpu_energy(inp)
+    assert_parity(E, lo, Eo, loo)
+    from paper_2209_04015_b200 import LocalEnergy  # noqa: F401  (force-bias check on the complex path too)
+    le = _le(inp)
+    gpu_energy(inp, le)
+    fb = le.force_bias(nw)
+    torch.cuda.synchronize()
+    ref = orc.force_bias(inp.chol, inp.psi_a, inp.psi_b, inp.phi_a[0], inp.phi_b[0])
+    assert np.all(np.abs(fb.cpu().numpy()[0] - ref) <= 1e-10 * np.max(np.abs(ref)))
+    le.close()
 
 
 def test_fewer_walkers_than_capacity_and_ragged_tail():
@@ -185,8 +215,8 @@ def test_errors_are_reported():
     dev = "cuda"
     h, c = torch.from_numpy(inp.h1e).to(dev), torch.from_numpy(inp.chol).to(dev)
     t = torch.from_numpy(inp.trial_packed()).to(dev)
-    with pytest.raises(AfqmcError, match="imaginary"):
-        LocalEnergy(h, c, t * (1 + 0.1j), inp.N, 3, 3, inp.n_gamma, 0.0, 4)
+    with pytest.raises(AfqmcError, match="non-finite"):
+        LocalEnergy(h, c, t * float("nan"), inp.N, 3, 3, inp.n_gamma, 0.0, 4)
     with pytest.raises(AfqmcError, match="out of range"):
         LocalEnergy(h, c, t, inp.N, 3, 3, inp.n_gamma, 0.0, 0)
     le = LocalEnergy(h, c, t, inp.N, 3, 3, inp.n_gamma, 0.0, 2)
