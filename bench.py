@@ -195,6 +195,7 @@ def main():
     chol = torch.from_numpy(inp.chol).to(dev)
     trial = torch.from_numpy(inp.trial_packed()).to(dev)
     le = LocalEnergy(h1e, chol, trial, inp.N, inp.n_alpha, inp.n_beta, inp.n_gamma, inp.e0, nw)
+    le.enable_force_bias(chol)          # operand of the dedicated force-bias GEMM (reported under "force_bias")
     del chol
     torch.cuda.empty_cache()
     walkers_host = torch.from_numpy(inp.walkers_packed()).pin_memory()
@@ -245,6 +246,19 @@ def main():
     ms_e2e = max_over_ranks(e0.elapsed_time(e1))
     e2e_value = world * nw * args.steps / (ms_e2e * 1e-3)
     same = bool(torch.equal(outE_h.view(torch.float64), outE.cpu().view(torch.float64)))
+
+    # ---- the force bias without the energy: K1 + one DMMA GEMM per spin + combine ------------------
+    fb_out = torch.empty((nw, inp.n_gamma), dtype=torch.complex128, device=dev)
+    for _ in range(3):
+        le.force_bias_only(walkers, nw, fb_out)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        le.force_bias_only(walkers, nw, fb_out)
+    e1.record(stream)
+    barrier()
+    ms_fb = max_over_ranks(e0.elapsed_time(e1)) / args.steps
+    flops_fb = 4.0 * inp.N * inp.n_gamma * nw * (inp.n_alpha + inp.n_beta)
 
     # ---- roofline of K2 -------------------------------------------------------------------------------------
     nspin_launches = int(inp.n_alpha > 0) + int(inp.n_beta > 0)
@@ -354,6 +368,12 @@ def main():
                         "d2h_bytes_per_step": int(2 * nw * 16), "ms_per_step": ms_e2e / args.steps,
                         "matches_device_path_bitwise": same},
                 "gpu_launches": int(gpu_launches),
+                "force_bias": {"value": world * nw / (ms_fb * 1e-3), "unit": UNIT, "ms_per_step": ms_fb,
+                               "what": "afqmc_force_bias_only: K1 + [Ngamma x nN].[nN x 2Nw] DMMA GEMM per spin + "
+                                       "combine; device-resident, same walkers",
+                               "algorithmic_flops_per_step": flops_fb,
+                               "tflops_incl_k1": flops_fb / (ms_fb * 1e-3) * 1e-12,
+                               "speedup_vs_energy_step": (ms_total / args.steps) / ms_fb},
                 "roofline": roofline,
                 "cpu_baseline": cpu}
         if others is not None:

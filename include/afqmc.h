@@ -98,6 +98,23 @@ int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walk
  */
 int afqmc_force_bias(afqmc_ctx *ctx, void *out, void *stream);
 
+/*
+ * afqmc_enable_force_bias / afqmc_force_bias_only -- the force bias WITHOUT the energy, for the propagation steps
+ * between energy evaluations (25 per block in the paper's runs):
+ *     xbar^gamma_w = sum_sigma sum_ip Ltilde^gamma_ip theta_ip           PAPER.md:195 (Eq. 24), Listing 3
+ * i.e. one real GEMM [Ngamma x n N] . [n N x 2 Nw] per spin (re and im planes of theta as columns) on the FP64 tensor
+ * cores, after K1 has built theta.
+ *   afqmc_enable_force_bias builds a second copy of Ltilde in that GEMM's operand order (about the size of the first:
+ *   Ngamma * n * N doubles per spin, twice that for a complex trial block) from `chol` (device, the array given to
+ *   afqmc_create, not retained) and synchronises `stream`.  Idempotent.
+ *   afqmc_force_bias_only enqueues K1, the GEMM (one launch per spin) and a combine kernel on `stream`:
+ *     walkers  device, layout as in afqmc_local_energy;  n_walkers 1 .. max_walkers
+ *     out      device, complex128 [n_walkers][n_gamma]
+ *   Returns AFQMC_ERR_ARG if afqmc_enable_force_bias has not been called on this handle.
+ */
+int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream);
+int afqmc_force_bias_only(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out, void *stream);
+
 /* Frees the handle and every internal buffer.  NULL is allowed. */
 void afqmc_destroy(afqmc_ctx *ctx);
 

@@ -13,7 +13,8 @@ import torch
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
-EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias", "afqmc_destroy",
+EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias",
+           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
            "afqmc_fp64_peak", "afqmc_plan"]
 
@@ -53,6 +54,10 @@ def load_library():
     lib.afqmc_local_energy_host.restype = ip
     lib.afqmc_force_bias.argtypes = [vp, vp, vp]
     lib.afqmc_force_bias.restype = ip
+    lib.afqmc_enable_force_bias.argtypes = [vp, vp, vp]
+    lib.afqmc_enable_force_bias.restype = ip
+    lib.afqmc_force_bias_only.argtypes = [vp, vp, ip, vp, vp]
+    lib.afqmc_force_bias_only.restype = ip
     lib.afqmc_destroy.argtypes = [vp]
     lib.afqmc_destroy.restype = None
     lib.afqmc_last_error.argtypes = [vp]
@@ -174,6 +179,26 @@ class LocalEnergy:
         if out is None:
             out = torch.empty((n_walkers, self.n_gamma), dtype=torch.complex128, device="cuda")
         self._check(self._lib.afqmc_force_bias(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_force_bias")
+        return out
+
+    def enable_force_bias(self, chol, stream=None):
+        """afqmc_enable_force_bias: build the operand of the dedicated force-bias GEMM from ``chol`` (CUDA float64)."""
+        if not (chol.is_cuda and chol.is_contiguous() and chol.dtype == torch.float64) or \
+                chol.numel() != self.n_gamma * self.N * self.N:
+            raise AfqmcError("chol must be the contiguous CUDA float64 [n_gamma, N, N] tensor given at creation")
+        self._check(self._lib.afqmc_enable_force_bias(self._h, chol.data_ptr(), _stream_ptr(stream)),
+                    "afqmc_enable_force_bias")
+
+    def force_bias_only(self, walkers, n_walkers, out=None, stream=None):
+        """afqmc_force_bias_only: [n_walkers, n_gamma] complex128 force bias without the energy."""
+        if not (walkers.is_cuda and walkers.is_contiguous() and walkers.dtype == torch.complex128):
+            raise AfqmcError("walkers must be a contiguous CUDA complex128 tensor")
+        if walkers.numel() != n_walkers * self.N * (self.n_alpha + self.n_beta):
+            raise AfqmcError("walkers has the wrong number of elements")
+        if out is None:
+            out = torch.empty((n_walkers, self.n_gamma), dtype=torch.complex128, device=walkers.device)
+        self._check(self._lib.afqmc_force_bias_only(self._h, walkers.data_ptr(), n_walkers, out.data_ptr(),
+                                                    _stream_ptr(stream)), "afqmc_force_bias_only")
         return out
 
     def info(self) -> dict:

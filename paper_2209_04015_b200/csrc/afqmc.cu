@@ -38,6 +38,11 @@ struct SpinCfg {
     double *psi_im = nullptr, *ht_im = nullptr;   // complex trial only
     int nb = 0;                                   // rows of one gamma block of the A operand: n (real trial) or 2n
     bool cplx = false;                            // this spin's trial block has a non-zero imaginary part
+    // dedicated force-bias path (afqmc_enable_force_bias): operands packed with n = 1, k = (i, p)
+    int f_gT = 0, f_wT = 0, f_NT = 0, f_strips = 0, f_ksteps = 0, f_ksc = 0, f_nchunks = 0, f_nstages = 0, f_n_rt = 0, f_n_ct_max = 0, f_ksplit = 1, f_kps = 0;
+    size_t f_smem = 0;
+    OperandLayout f_layA{}, f_layB{};
+    double *f_A = nullptr, *f_B = nullptr, *f_craw = nullptr;
     size_t A_bytes = 0, B_bytes = 0;
 };
 
@@ -53,6 +58,7 @@ struct afqmc_ctx {
     double2 *h_walkers = nullptr;      // device staging for the host-buffer entry point
     double *h_outE = nullptr, *h_outO = nullptr;
     int last_nw = 0;
+    bool fb_enabled = false;
     long long launches = 0;
     bool profiling = false;
     std::vector<cudaEvent_t> ev;       // kProfSets x 4 events, created by the first afqmc_set_profiling(1)
@@ -196,10 +202,23 @@ K2Fn k2_pick(int mt, int nt) {
     return nullptr;
 }
 
+using K2FbFn = void (*)(const K2FbParams);
+template <int NT>
+K2FbFn k2_pick_fb_nt(int nt) {
+    if constexpr (NT == 0) {
+        return nullptr;
+    } else {
+        if (nt == NT) return k2_force_bias<NT>;
+        return k2_pick_fb_nt<NT - 1>(nt);
+    }
+}
+K2FbFn k2_pick_fb(int nt) { return k2_pick_fb_nt<16>(nt); }
+
 void free_ctx(afqmc_ctx *c) {
     if (!c) return;
     for (int s = 0; s < 2; ++s) {
         cudaFree(c->sp[s].A); cudaFree(c->sp[s].B); cudaFree(c->sp[s].psi); cudaFree(c->sp[s].ht); cudaFree(c->sp[s].psi_im); cudaFree(c->sp[s].ht_im);
+        cudaFree(c->sp[s].f_A); cudaFree(c->sp[s].f_B); cudaFree(c->sp[s].f_craw);
         cudaFree(c->sp[s].tbuf); cudaFree(c->sp[s].xpart);
     }
     cudaFree(c->e1); cudaFree(c->logdet); cudaFree(c->h_walkers); cudaFree(c->h_outE); cudaFree(c->h_outO);
@@ -215,6 +234,29 @@ int check_arch(afqmc_ctx *ctx, int *num_sms) {
     CU_TRY(ctx, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     if (major != 10) return fail(ctx, AFQMC_ERR_ARCH, "device compute capability %d.x is not sm_100", major);
     if (num_sms) *num_sms = sms;
+    return AFQMC_OK;
+}
+
+// K1 for `n_walkers` walkers; with_fb also writes theta in the force-bias operand order.
+int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, cudaStream_t stream) {
+    const int N = ctx->N;
+    K1Params p1{};
+    p1.walkers = reinterpret_cast<const double2 *>(walkers);
+    p1.n_walkers = n_walkers; p1.N = N; p1.maxw = ctx->maxw;
+    p1.spin_off[0] = 0;
+    p1.spin_off[1] = (long long)n_walkers * N * ctx->sp[0].n;
+    for (int s = 0; s < 2; ++s) {
+        p1.n[s] = ctx->sp[s].n; p1.psi[s] = ctx->sp[s].psi; p1.ht[s] = ctx->sp[s].ht;
+        p1.psi_im[s] = ctx->sp[s].psi_im; p1.ht_im[s] = ctx->sp[s].ht_im;
+        p1.thetaB[s] = ctx->sp[s].B; p1.layB[s] = ctx->sp[s].layB;
+        p1.thetaF[s] = with_fb ? ctx->sp[s].f_B : nullptr; p1.layF[s] = ctx->sp[s].f_layB;
+    }
+    p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
+    size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
+    if (with_fb) k1_overlap_inverse_theta<true><<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
+    else k1_overlap_inverse_theta<false><<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
     return AFQMC_OK;
 }
 
@@ -297,13 +339,13 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         dim3 grid((N + 127) / 128, n_gamma);
         k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi, N, n, 1.0, sc.ht);
         CR_TRY(cudaGetLastError());
-        k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, sc.nb, 0, 1.0, sc.layA, sc.A);
+        k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, sc.nb, 0, 1.0, sc.layA, sc.A, OperandLayout{}, nullptr);
         CR_TRY(cudaGetLastError());
         c->launches += 2;
         if (cplx) {                                   // conj(psi) = Re psi - i Im psi
             k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi_im, N, n, -1.0, sc.ht_im);
             CR_TRY(cudaGetLastError());
-            k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi_im, N, n, n_gamma, sc.nb, n, -1.0, sc.layA, sc.A);
+            k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi_im, N, n, n_gamma, sc.nb, n, -1.0, sc.layA, sc.A, OperandLayout{}, nullptr);
             CR_TRY(cudaGetLastError());
             c->launches += 2;
         }
@@ -315,7 +357,8 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         CR_TRY(cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc.k2_smem));
     }
     size_t k1s = std::max(c->sp[0].k1_smem, c->sp[1].k1_smem);
-    CR_TRY(cudaFuncSetAttribute((const void *)k1_overlap_inverse_theta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k1s));
+    CR_TRY(cudaFuncSetAttribute((const void *)k1_overlap_inverse_theta<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k1s));
+    CR_TRY(cudaFuncSetAttribute((const void *)k1_overlap_inverse_theta<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k1s));
     CR_TRY(cudaMalloc(&c->e1, (size_t)2 * max_walkers * 16));
     CR_TRY(cudaMalloc(&c->logdet, (size_t)2 * max_walkers * 16));
     CR_TRY(cudaMemsetAsync(c->e1, 0, (size_t)2 * max_walkers * 16, stream));
@@ -341,21 +384,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     if (ev) CU_TRY(ctx, cudaEventRecord(ev[0], stream));
 
     // ---- K1 -------------------------------------------------------------------------------------------
-    K1Params p1{};
-    p1.walkers = reinterpret_cast<const double2 *>(walkers);
-    p1.n_walkers = n_walkers; p1.N = N; p1.maxw = ctx->maxw;
-    p1.spin_off[0] = 0;
-    p1.spin_off[1] = (long long)n_walkers * N * ctx->sp[0].n;
-    for (int s = 0; s < 2; ++s) {
-        p1.n[s] = ctx->sp[s].n; p1.psi[s] = ctx->sp[s].psi; p1.ht[s] = ctx->sp[s].ht;
-        p1.psi_im[s] = ctx->sp[s].psi_im; p1.ht_im[s] = ctx->sp[s].ht_im;
-        p1.thetaB[s] = ctx->sp[s].B; p1.layB[s] = ctx->sp[s].layB;
-    }
-    p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
-    size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
-    k1_overlap_inverse_theta<<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
-    CU_TRY(ctx, cudaGetLastError());
-    ctx->launches += 1;
+    if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream)) return rc;
     if (ev) CU_TRY(ctx, cudaEventRecord(ev[1], stream));
 
     // ---- K2, once per spin ------------------------------------------------------------------------------
@@ -420,6 +449,108 @@ int afqmc_force_bias(afqmc_ctx *ctx, void *out, void *stream_) {
     const long long total = (long long)ctx->last_nw * ctx->n_gamma * 2;
     k3_force_bias<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream_>>>(
         ctx->last_nw, ctx->n_gamma, ctx->sp[0].n, ctx->sp[1].n, ctx->sp[0].tbuf, ctx->sp[1].tbuf, reinterpret_cast<double *>(out));
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!chol) return fail(ctx, AFQMC_ERR_ARG, "afqmc_enable_force_bias: null pointer argument");
+    if (ctx->fb_enabled) return AFQMC_OK;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int N = ctx->N, n_gamma = ctx->n_gamma, maxw = ctx->maxw;
+    for (int s = 0; s < 2; ++s) {
+        SpinCfg &sc = ctx->sp[s];
+        const int n = sc.n;
+        if (n == 0) continue;
+        const int nbf = sc.cplx ? 2 : 1;                          // rows per gamma: Re (and Im) of Ltilde
+        sc.f_wT = std::min(64, (maxw + 3) / 4 * 4);               // 2 * wT columns = 8 * NT
+        sc.f_NT = sc.f_wT / 4;
+        sc.f_strips = std::min(K2_MAX_WM, (n_gamma * nbf + 7) / 8);
+        sc.f_gT = sc.f_strips * 8 / nbf;
+        sc.f_n_rt = (n_gamma + sc.f_gT - 1) / sc.f_gT;
+        sc.f_n_ct_max = (maxw + sc.f_wT - 1) / sc.f_wT;
+        // split K so that (row tiles x column tiles x K parts) fills whole rounds of the persistent grid
+        const int ks_raw = (n * N + 3) / 4;
+        sc.f_ksc = std::min(4, ks_raw);
+        int best_s = 1;
+        double best_fill = 0.0;
+        for (int sp = 1; sp <= 8; ++sp) {
+            if (ks_raw / sp < 4 * sc.f_ksc && sp > 1) break;     // keep every part at least a few chunks long
+            const long long items = (long long)sc.f_n_rt * sc.f_n_ct_max * sp;
+            const long long rounds = (items + ctx->num_sms - 1) / ctx->num_sms;
+            const double fill = (double)items / (double)(rounds * ctx->num_sms);
+            if (fill > best_fill + 0.02) { best_fill = fill; best_s = sp; }
+        }
+        sc.f_ksplit = best_s;
+        sc.f_kps = ((ks_raw + best_s - 1) / best_s + sc.f_ksc - 1) / sc.f_ksc * sc.f_ksc;   // k-steps per part, whole chunks
+        sc.f_ksteps = sc.f_kps * best_s;                                                   // padded with zero k-steps
+        sc.f_nchunks = sc.f_kps / sc.f_ksc;
+        sc.f_nstages = 5;
+        sc.f_smem = (size_t)sc.f_nstages * sc.f_ksc * (sc.f_strips + sc.f_NT) * 256 + (size_t)2 * sc.f_nstages * 8 + 16;
+        sc.f_layA = OperandLayout{1, sc.f_strips, sc.f_ksteps, sc.f_gT, (long long)sc.f_strips * sc.f_ksteps * 32};
+        sc.f_layB = OperandLayout{1, sc.f_NT, sc.f_ksteps, sc.f_wT, (long long)sc.f_NT * sc.f_ksteps * 32};
+        const size_t a_bytes = (size_t)sc.f_n_rt * sc.f_layA.tile_doubles * 8, b_bytes = (size_t)sc.f_n_ct_max * sc.f_layB.tile_doubles * 8;
+        const size_t c_bytes = (size_t)sc.f_ksplit * n_gamma * nbf * sc.f_n_ct_max * sc.f_NT * 8 * 8;
+        CU_TRY(ctx, cudaMalloc(&sc.f_A, a_bytes));
+        CU_TRY(ctx, cudaMalloc(&sc.f_B, b_bytes));
+        CU_TRY(ctx, cudaMalloc(&sc.f_craw, c_bytes));
+        CU_TRY(ctx, cudaMemsetAsync(sc.f_A, 0, a_bytes, stream));
+        CU_TRY(ctx, cudaMemsetAsync(sc.f_B, 0, b_bytes, stream));
+        dim3 grid((N + 127) / 128, n_gamma);
+        k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, n * nbf, 0, 1.0, OperandLayout{}, nullptr, sc.f_layA, sc.f_A);
+        CU_TRY(ctx, cudaGetLastError());
+        ctx->launches += 1;
+        if (sc.cplx) {
+            k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi_im, N, n, n_gamma, n * nbf, n, -1.0, OperandLayout{}, nullptr, sc.f_layA, sc.f_A);
+            CU_TRY(ctx, cudaGetLastError());
+            ctx->launches += 1;
+        }
+        K2FbFn fn = k2_pick_fb(sc.f_NT);
+        if (!fn) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_enable_force_bias: no kernel for NT=%d", sc.f_NT);
+        CU_TRY(ctx, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc.f_smem));
+    }
+    CU_TRY(ctx, cudaStreamSynchronize(stream));
+    ctx->fb_enabled = true;
+    return AFQMC_OK;
+}
+
+int afqmc_force_bias_only(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!walkers || !out) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias_only: null pointer argument");
+    if (!ctx->fb_enabled) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias_only: call afqmc_enable_force_bias first");
+    if (n_walkers < 1 || n_walkers > ctx->maxw)
+        return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias_only: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (int rc = launch_k1(ctx, walkers, n_walkers, true, stream)) return rc;
+    K4Params p4{};
+    p4.n_walkers = n_walkers; p4.n_gamma = ctx->n_gamma; p4.out = reinterpret_cast<double *>(out);
+    for (int s = 0; s < 2; ++s) {
+        const SpinCfg &sc = ctx->sp[s];
+        p4.n[s] = sc.n;
+        if (sc.n == 0) continue;
+        const int nbf = sc.cplx ? 2 : 1;
+        K2FbParams p2{};
+        p2.A = sc.f_A; p2.B = sc.f_B;
+        p2.itemA_doubles = sc.f_layA.tile_doubles / sc.f_ksplit;   // parts of a tile are contiguous
+        p2.tileB_doubles = sc.f_layB.tile_doubles;
+        p2.partB_doubles = (long long)sc.f_kps * sc.f_NT * 32;
+        p2.rows_per_tile = sc.f_gT * nbf; p2.rows_total = ctx->n_gamma * nbf;
+        p2.strips = sc.f_strips; p2.WM = K2_MAX_WM;
+        p2.kps = sc.f_kps; p2.ksc = sc.f_ksc; p2.nchunks = sc.f_nchunks; p2.nstages = sc.f_nstages;
+        p2.n_items_r = sc.f_n_rt * sc.f_ksplit; p2.ksplit = sc.f_ksplit; p2.n_ct = (n_walkers + sc.f_wT - 1) / sc.f_wT;
+        p2.craw = sc.f_craw;
+        const long long ntiles = (long long)p2.n_items_r * p2.n_ct;
+        const int grid = (int)std::min<long long>(ntiles, ctx->num_sms);
+        K2FbFn fn = k2_pick_fb(sc.f_NT);
+        fn<<<grid, 32 * K2_MAX_WM, sc.f_smem, stream>>>(p2);
+        CU_TRY(ctx, cudaGetLastError());
+        ctx->launches += 1;
+        p4.nb[s] = nbf; p4.wT[s] = sc.f_wT; p4.n_ct[s] = p2.n_ct; p4.ldc[s] = sc.f_NT * 8; p4.craw[s] = sc.f_craw; p4.ksplit[s] = sc.f_ksplit;
+    }
+    const long long total = (long long)n_walkers * ctx->n_gamma;
+    k4_force_bias_combine<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(p4);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;

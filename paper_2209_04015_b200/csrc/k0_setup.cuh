@@ -26,7 +26,11 @@ constexpr int K0_PCHUNK = 64;
 
 __global__ void __launch_bounds__(128)
 k0_half_rotate_chol(const double *__restrict__ chol, const double *__restrict__ psi, int N, int n, int n_gamma,
-                    int rows_per_gamma, int row_shift, double scale, OperandLayout lay, double *__restrict__ packedA) {
+                    int rows_per_gamma, int row_shift, double scale, OperandLayout lay, double *__restrict__ packedA,
+                    OperandLayout layF, double *__restrict__ packedF) {
+    // packedA (may be null): K2's exchange operand, rows (gamma, [part,] i), k = p.
+    // packedF (may be null): the force-bias operand, rows (gamma[, part]), k = i * N + p   (Eq. 24).
+    const int nbf = rows_per_gamma / n, part = row_shift / n;
     __shared__ double psi_s[K0_PCHUNK * 8];  // [K0_PCHUNK][8]
     const int g = blockIdx.y;
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
@@ -56,7 +60,13 @@ k0_half_rotate_chol(const double *__restrict__ chol, const double *__restrict__ 
         if (r < N) {
 #pragma unroll
             for (int k = 0; k < 8; ++k)
-                if (i0 + k < n) packedA[packed_offset(lay, tile, row0 + i0 + k, r)] = scale * acc[k];
+                if (i0 + k < n) {
+                    if (packedA) packedA[packed_offset(lay, tile, row0 + i0 + k, r)] = scale * acc[k];
+                    if (packedF) {
+                        const int tf = g / layF.per_tile;
+                        packedF[packed_offset(layF, tf, (g - tf * layF.per_tile) * nbf + part, (i0 + k) * N + r)] = scale * acc[k];
+                    }
+                }
         }
     }
 }

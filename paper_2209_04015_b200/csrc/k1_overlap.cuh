@@ -26,6 +26,8 @@ struct K1Params {
     const double *ht_im[2];       // Im htilde, or nullptr
     double *thetaB[2];            // packed B operand
     OperandLayout layB[2];
+    double *thetaF[2];            // force-bias B operand (k = j * N + p, column = plane * wT + wl), or nullptr
+    OperandLayout layF[2];
     double *logdet;               // [2][maxw][2]  (log|det|, arg)
     double *e1;                   // [2][maxw][2]
 };
@@ -34,6 +36,7 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
     return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
+template <bool WITH_FB>
 __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params P) {
     const int w = blockIdx.x, sp = blockIdx.y;
     const int n = P.n[sp], N = P.N;
@@ -194,6 +197,9 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
     const int tile = w / wT, wl = w - tile * wT;
     const int col_re = wl * n, col_im = (wT + wl) * n;
     double *out = P.thetaB[sp];
+    double *outF = WITH_FB ? P.thetaF[sp] : nullptr;
+    const OperandLayout layF = P.layF[sp];
+    const int tileF = WITH_FB ? w / layF.per_tile : 0, wlF = WITH_FB ? w - tileF * layF.per_tile : 0;
     const double *ht = P.ht[sp];
     const double *ht_im = P.ht_im[sp];
     const int kk = lane & 3, jj = lane >> 2;
@@ -227,6 +233,10 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
                 }
                 out[packed_offset(lay, tile, col_re + j, p)] = acc.x;
                 out[packed_offset(lay, tile, col_im + j, p)] = acc.y;
+                if (WITH_FB && p < N) {
+                    outF[packed_offset(layF, tileF, wlF, j * N + p)] = acc.x;
+                    outF[packed_offset(layF, tileF, layF.per_tile + wlF, j * N + p)] = acc.y;
+                }
             }
         }
     }

@@ -339,4 +339,100 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
     else run_tiles(std::integral_constant<int, MT - 1>{});
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Force-bias GEMM (Eq. 24; Listing 3): xbar^gamma_w = sum_ip Ltilde^gamma_ip theta^w_ip.
+// Same operand ring and K loop as the exchange kernel, with the operands packed for n = 1 and k = (i, p): rows are
+// gamma (x Re/Im of Ltilde for a complex trial), columns are (plane, walker), every warp owns one 8-row strip and all NT
+// column blocks.  The K range is cut into `ksplit` equal parts so that (row tile, K part, column tile) items fill whole
+// rounds of the persistent grid; every accumulator element is stored raw and `k4_force_bias_combine` adds the parts in
+// a fixed order.
+struct K2FbParams {
+    const double *A, *B;           // packed operands (common.cuh), k-steps per tile = ksplit * kps
+    long long itemA_doubles;       // one (row tile, K part) of A: kps * strips * 32
+    long long tileB_doubles;       // one column tile of B, all K parts
+    long long partB_doubles;       // one K part of a B tile: kps * NT * 32
+    int rows_per_tile, rows_total; // valid rows per row tile, n_gamma * nb
+    int strips, WM;
+    int kps, ksc, nchunks, nstages;
+    int n_items_r;                 // row tiles * ksplit
+    int ksplit, n_ct;
+    double *craw;                  // [ksplit][rows_total][n_ct][8 * NT]
+};
+
+template <int NT>
+__global__ void __launch_bounds__(32 * K2_MAX_WM) k2_force_bias(const K2FbParams P) {
+    extern __shared__ __align__(128) unsigned char k2_smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int WM = P.WM;
+    const uint32_t a_chunk_bytes = (uint32_t)P.ksc * P.strips * 256u;
+    const uint32_t b_chunk_bytes = (uint32_t)P.ksc * NT * 256u;
+    const uint32_t stage_bytes = a_chunk_bytes + b_chunk_bytes;
+    unsigned char *stage_base = k2_smem;
+    uint64_t *full_bar = reinterpret_cast<uint64_t *>(k2_smem + (size_t)P.nstages * stage_bytes);
+    uint64_t *empty_bar = full_bar + P.nstages;
+    const int mma_warps = min(WM, P.strips);
+    if (tid == 0) {
+        for (int s = 0; s < P.nstages; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], mma_warps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (warp >= mma_warps) return;                       // no strip, no barrier duty
+
+    const int step_rt = (int)(gridDim.x / (unsigned)P.n_ct), step_ct = (int)(gridDim.x % (unsigned)P.n_ct);
+    const int first_rt = (int)(blockIdx.x / (unsigned)P.n_ct), first_ct = (int)(blockIdx.x % (unsigned)P.n_ct);
+
+    const bool producer_warp = (warp == mma_warps - 1);
+    int p_rt = first_rt, p_ct = first_ct, p_chunk = 0, p_stage = 0;
+    uint32_t p_phase = 0;
+    const double *p_a = P.A + (long long)p_rt * P.itemA_doubles;
+    const double *p_b = P.B + (long long)p_ct * P.tileB_doubles + (p_rt % P.ksplit) * P.partB_doubles;
+    auto produce_poll = [&]() {
+        if (p_rt >= P.n_items_r) return;
+        if (!mbar_test_addr(smem_u32(&empty_bar[p_stage]), p_phase ^ 1u)) return;
+        mbar_arrive_expect_tx(&full_bar[p_stage], a_chunk_bytes + b_chunk_bytes);
+        unsigned char *dst = stage_base + (size_t)p_stage * stage_bytes;
+        bulk_g2s(dst, p_a, a_chunk_bytes, &full_bar[p_stage]);
+        bulk_g2s(dst + a_chunk_bytes, p_b, b_chunk_bytes, &full_bar[p_stage]);
+        p_a += a_chunk_bytes / 8; p_b += b_chunk_bytes / 8;
+        if (++p_stage == P.nstages) { p_stage = 0; p_phase ^= 1u; }
+        if (++p_chunk == P.nchunks) {
+            p_chunk = 0;
+            p_rt += step_rt; p_ct += step_ct;
+            if (p_ct >= P.n_ct) { p_ct -= P.n_ct; ++p_rt; }
+            p_a = P.A + (long long)p_rt * P.itemA_doubles;
+            p_b = P.B + (long long)p_ct * P.tileB_doubles + (p_rt % P.ksplit) * P.partB_doubles;
+        }
+    };
+    if (producer_warp && lane == 0)
+        for (int d = 0; d < P.nstages; ++d) produce_poll();
+
+    K2Ring R;
+    R.smem_base = smem_u32(stage_base); R.stage_bytes = stage_bytes; R.a_chunk_bytes = a_chunk_bytes;
+    R.a_kstride = (uint32_t)P.strips * 256u;
+    R.full_bar = smem_u32(full_bar); R.empty_bar = smem_u32(empty_bar);
+    R.nstages = P.nstages; R.ksc = P.ksc; R.nchunks = P.nchunks; R.last_ks = P.ksc; R.ksteps = P.kps;   // whole chunks only
+    R.stage = 0; R.phase = 0;
+    const uint32_t frag_off = (uint32_t)warp * 256u + 8u * lane;
+
+    for (int rt = first_rt, ct = first_ct; rt < P.n_items_r;) {
+        double acc[1][NT][2];
+#pragma unroll
+        for (int q = 0; q < NT; ++q) { acc[0][q][0] = 0.0; acc[0][q][1] = 0.0; }
+        k2_tile_mma<1, NT>(acc, R, frag_off, 0u, producer_warp, produce_poll, lane);
+        const int rtile = rt / P.ksplit, part = rt - rtile * P.ksplit;
+        const int lrow = warp * 8 + (lane >> 2);
+        const int row = rtile * P.rows_per_tile + lrow;
+        if (lrow < P.rows_per_tile && row < P.rows_total) {
+            double *dst = P.craw + (((long long)part * P.rows_total + row) * P.n_ct + ct) * (NT * 8) + 2 * (lane & 3);
+#pragma unroll
+            for (int q = 0; q < NT; ++q) *reinterpret_cast<double2 *>(dst + q * 8) = make_double2(acc[0][q][0], acc[0][q][1]);
+        }
+        rt += step_rt; ct += step_ct;
+        if (ct >= P.n_ct) { ct -= P.n_ct; ++rt; }
+    }
+}
+
 }  // namespace afqmc

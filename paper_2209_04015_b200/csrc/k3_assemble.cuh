@@ -80,4 +80,37 @@ __global__ void k3_force_bias(int n_walkers, int n_gamma, int na, int nb, const 
     out[idx] = v;
 }
 
+// force bias from the raw products of K2's force-bias mode          PAPER.md:168-170, 195 (Eq. 19, 24)
+//   real Ltilde:     xbar = (C[gamma][re w], C[gamma][im w])
+//   complex Ltilde:  xbar = (C[re gamma][re w] - C[im gamma][im w],  C[re gamma][im w] + C[im gamma][re w])
+struct K4Params {
+    int n_walkers, n_gamma;
+    int n[2], nb[2], wT[2], n_ct[2], ldc[2];   // nb = rows per gamma (1 or 2), ldc = 8 * NT columns per tile
+    int ksplit[2];                              // K parts, summed here in a fixed order
+    const double *craw[2];
+    double *out;                                // [n_walkers][n_gamma][2]
+};
+
+__global__ void k4_force_bias_combine(K4Params P) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)P.n_walkers * P.n_gamma) return;
+    const int w = (int)(idx / P.n_gamma), g = (int)(idx - (long long)w * P.n_gamma);
+    double xr = 0.0, xi = 0.0;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        if (P.n[s] == 0) continue;
+        const int ct = w / P.wT[s], wl = w - ct * P.wT[s];
+        const long long part_stride = (long long)P.n_gamma * P.nb[s] * P.n_ct[s] * P.ldc[s];
+        for (int k = 0; k < P.ksplit[s]; ++k) {
+            const double *c0 = P.craw[s] + k * part_stride + ((long long)(g * P.nb[s]) * P.n_ct[s] + ct) * P.ldc[s];
+            xr += c0[wl]; xi += c0[P.wT[s] + wl];
+            if (P.nb[s] == 2) {
+                const double *c1 = c0 + (long long)P.n_ct[s] * P.ldc[s];
+                xr -= c1[P.wT[s] + wl]; xi += c1[wl];
+            }
+        }
+    }
+    P.out[2 * idx] = xr; P.out[2 * idx + 1] = xi;
+}
+
 }  // namespace afqmc

@@ -209,6 +209,37 @@ def test_host_entry_point_and_force_bias():
     le.close()
 
 
+@pytest.mark.parametrize("case", ["small", "ragged", "complex", "one_spin"])
+def test_force_bias_only_matches_oracle_and_energy_path(case):
+    """Dedicated force-bias GEMM (afqmc_force_bias_only) against sum_pq G_pq L^gamma_pq from the full Green's
+    function (Eq. 19), and against the traces the energy path produces."""
+    if case == "small":
+        inp = make_inputs("small", n_walkers=70, n_gamma=130)      # two walker tiles (64 + 6), two gamma tiles
+    elif case == "ragged":
+        inp = _custom(411, 33, 13, 11, 101, 7)
+    elif case == "complex":
+        inp = _custom(412, 21, 6, 5, 50, 9, complex_trial="both")
+    else:
+        inp = _custom(413, 10, 4, 0, 9, 3)
+    le = _le(inp)
+    from paper_2209_04015_b200 import AfqmcError
+    w = torch.from_numpy(inp.walkers_packed()).cuda()
+    with pytest.raises(AfqmcError, match="afqmc_enable_force_bias"):
+        le.force_bias_only(w, inp.n_walkers)
+    le.enable_force_bias(torch.from_numpy(inp.chol).cuda())
+    fb = le.force_bias_only(w, inp.n_walkers)
+    torch.cuda.synchronize()
+    fb = fb.cpu().numpy()
+    for k in sorted({0, inp.n_walkers // 2, inp.n_walkers - 1}):
+        ref = orc.force_bias(inp.chol, inp.psi_a, inp.psi_b, inp.phi_a[k], inp.phi_b[k])
+        assert np.all(np.abs(fb[k] - ref) <= 1e-10 * np.max(np.abs(ref))), k
+    le.local_energy(w, inp.n_walkers)
+    fb2 = le.force_bias(inp.n_walkers)
+    torch.cuda.synchronize()
+    assert np.all(np.abs(fb2.cpu().numpy() - fb) <= 1e-11 * np.max(np.abs(fb)))
+    le.close()
+
+
 def test_errors_are_reported():
     from paper_2209_04015_b200 import AfqmcError, LocalEnergy
     inp = make_inputs("tiny")
