@@ -319,3 +319,14 @@ def force_bias(chol, psi_a, psi_b, phi_a, phi_b):
     Ga, _, _ = greens_function(psi_a, phi_a)
     Gb, _, _ = greens_function(psi_b, phi_b)
     return np.einsum("gpq,pq->g", chol, Ga + Gb)
+
+
+def spin_squared(psi_a, psi_b, phi_a, phi_b):
+    """Mixed estimator <psi|S^2|phi>/<psi|phi> = N_dn + M_S (M_S + 1) - sum_pq G^dn_pq G^up_qp from the FULL Green's
+    functions (Eq. 31; the transposed index order is Listing 6's ``einsum("zij,zji->z", Ga, Gb)``,
+    PAPER.md:426, which is the correct Wick contraction of S_- S_+)."""
+    Ga, _, _ = greens_function(psi_a, phi_a)
+    Gb, _, _ = greens_function(psi_b, phi_b)
+    n_up, n_dn = psi_a.shape[1], psi_b.shape[1]
+    ms = 0.5 * (n_up - n_dn)
+    return n_dn + ms * (ms + 1.0) - np.einsum("ij,ji->", Ga, Gb)

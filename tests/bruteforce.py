@@ -115,3 +115,27 @@ def hartree_fock_energy_mo(h1e, chol, e0, psi_a, psi_b):
     for L in Lmo:
         e -= 0.5 * np.einsum("gij,gji->", L, L)                  # 1/2 sum_ij (ij|ji), equal spins
     return e
+
+
+def brute_force_spin_squared(psi_a, psi_b, phi_a, phi_b):
+    """<psi|S^2|phi>/<psi|phi> with S^2 = S_- S_+ + S_z (S_z + 1), S_+ = sum_p a+_{p,up} a_{p,dn}, applied operator by
+    operator to the determinant expansion of |phi> (no Green's function, no Wick's theorem).  alpha = up."""
+    N = psi_a.shape[0]
+    bits_phi, c_phi = _minor_expansion(phi_a, phi_b, N)
+    bits_psi, c_psi = _minor_expansion(psi_a, psi_b, N)
+    lookup = np.full(1 << (2 * N), -1, dtype=np.int64)
+    lookup[bits_psi] = np.arange(len(bits_psi))
+    phi_vec = np.zeros(len(bits_psi), dtype=np.complex128)
+    phi_vec[lookup[bits_phi]] = c_phi
+    ovlp = np.sum(np.conj(c_psi) * phi_vec)
+    bra = np.zeros(len(bits_psi), dtype=np.complex128)
+    for q in range(N):                      # S_+ = sum_q a+_{q,up} a_{q,dn}
+        b1, a1 = _annihilate(bits_phi, c_phi, N + q)
+        b2, a2 = _create(b1, a1, q)
+        for p in range(N):                  # S_- = sum_p a+_{p,dn} a_{p,up}
+            b3, a3 = _annihilate(b2, a2, p)
+            b4, a4 = _create(b3, a3, N + p)
+            if len(b4):
+                np.add.at(bra, lookup[b4], a4)
+    ms = 0.5 * (psi_a.shape[1] - psi_b.shape[1])
+    return np.sum(np.conj(c_psi) * bra) / ovlp + ms * (ms + 1.0)
