@@ -115,6 +115,15 @@ int afqmc_force_bias(afqmc_ctx *ctx, void *out, void *stream);
 int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream);
 int afqmc_force_bias_only(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out, void *stream);
 
+/*
+ * afqmc_spin_squared -- a second mixed estimator from the same half-rotated Green's function (Eq. 31
+ * with the index order of Listing 6):
+ *     s2_w = <psi_T|S^2|phi_w> / <psi_T|phi_w> = n_beta + M_S (M_S + 1) - sum_pq G^alpha_pq G^beta_qp ,   M_S = (n_alpha - n_beta) / 2
+ * for the walkers of the most recent afqmc_local_energy / afqmc_force_bias_only call (it reads the theta those calls
+ * left in the handle).  out: device, complex128 [n_walkers of that call].  Enqueued on `stream`.
+ */
+int afqmc_spin_squared(afqmc_ctx *ctx, void *out, void *stream);
+
 /* Frees the handle and every internal buffer.  NULL is allowed. */
 void afqmc_destroy(afqmc_ctx *ctx);
 

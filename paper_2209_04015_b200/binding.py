@@ -14,7 +14,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias",
-           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_destroy",
+           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
            "afqmc_fp64_peak", "afqmc_plan"]
 
@@ -58,6 +58,8 @@ def load_library():
     lib.afqmc_enable_force_bias.restype = ip
     lib.afqmc_force_bias_only.argtypes = [vp, vp, ip, vp, vp]
     lib.afqmc_force_bias_only.restype = ip
+    lib.afqmc_spin_squared.argtypes = [vp, vp, vp]
+    lib.afqmc_spin_squared.restype = ip
     lib.afqmc_destroy.argtypes = [vp]
     lib.afqmc_destroy.restype = None
     lib.afqmc_last_error.argtypes = [vp]
@@ -199,6 +201,14 @@ class LocalEnergy:
             out = torch.empty((n_walkers, self.n_gamma), dtype=torch.complex128, device=walkers.device)
         self._check(self._lib.afqmc_force_bias_only(self._h, walkers.data_ptr(), n_walkers, out.data_ptr(),
                                                     _stream_ptr(stream)), "afqmc_force_bias_only")
+        return out
+
+    def spin_squared(self, n_walkers, out=None, stream=None):
+        """afqmc_spin_squared: [n_walkers] complex128 <S^2> mixed estimator for the walkers of the last energy /
+        force-bias call."""
+        if out is None:
+            out = torch.empty(n_walkers, dtype=torch.complex128, device="cuda")
+        self._check(self._lib.afqmc_spin_squared(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_spin_squared")
         return out
 
     def info(self) -> dict:

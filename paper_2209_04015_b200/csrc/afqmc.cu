@@ -19,6 +19,7 @@
 #include "k1_overlap.cuh"
 #include "k2_exchange.cuh"
 #include "k3_assemble.cuh"
+#include "k5_spin_squared.cuh"
 
 using namespace afqmc;
 
@@ -551,6 +552,26 @@ int afqmc_force_bias_only(afqmc_ctx *ctx, const void *walkers, int n_walkers, vo
     }
     const long long total = (long long)n_walkers * ctx->n_gamma;
     k4_force_bias_combine<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(p4);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    ctx->last_nw = n_walkers;
+    return AFQMC_OK;
+}
+
+int afqmc_spin_squared(afqmc_ctx *ctx, void *out, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!out) return fail(ctx, AFQMC_ERR_ARG, "afqmc_spin_squared: null pointer argument");
+    if (ctx->last_nw < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_spin_squared: no energy or force-bias call has been made on this handle");
+    K5Params p5{};
+    p5.N = ctx->N; p5.n_walkers = ctx->last_nw; p5.out = reinterpret_cast<double *>(out);
+    for (int s = 0; s < 2; ++s) {
+        p5.n[s] = ctx->sp[s].n; p5.theta[s] = ctx->sp[s].B; p5.layB[s] = ctx->sp[s].layB;
+        p5.psi[s] = ctx->sp[s].psi; p5.psi_im[s] = ctx->sp[s].psi_im;
+    }
+    const int na = p5.n[0], nb = p5.n[1];
+    const size_t smem = ((size_t)2 * na * nb + (size_t)2 * (na + nb) * K5_PCHUNK) * 16;
+    CU_TRY(ctx, cudaFuncSetAttribute((const void *)k5_spin_squared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k5_spin_squared<<<ctx->last_nw, K5_THREADS, smem, (cudaStream_t)stream_>>>(p5);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;

@@ -240,6 +240,32 @@ def test_force_bias_only_matches_oracle_and_energy_path(case):
     le.close()
 
 
+@pytest.mark.parametrize("case", ["small", "uhf", "complex", "polarised", "big_n"])
+def test_spin_squared_matches_oracle(case):
+    """<S^2> mixed estimator (Eq. 31 / Listing 6) from the half-rotated Green's function against the
+    oracle's full-Green's-function einsum."""
+    if case == "small":
+        inp = make_inputs("small", n_walkers=9, n_gamma=20)            # RHF-style trial: a singlet, s2 = 0
+    elif case == "uhf":
+        inp = _custom(511, 33, 13, 11, 12, 6)
+    elif case == "complex":
+        inp = _custom(512, 21, 6, 5, 10, 5, complex_trial="both")
+    elif case == "polarised":
+        inp = _custom(513, 10, 4, 0, 9, 3)
+    else:
+        inp = _custom(514, 70, 64, 40, 6, 3)
+    le = _le(inp)
+    gpu_energy(inp, le)
+    s2 = le.spin_squared(inp.n_walkers)
+    torch.cuda.synchronize()
+    s2 = s2.cpu().numpy()
+    ref = np.array([orc.spin_squared(inp.psi_a, inp.psi_b, inp.phi_a[k], inp.phi_b[k]) for k in range(inp.n_walkers)])
+    assert np.all(np.abs(s2 - ref) <= 1e-10 * np.maximum(1.0, np.abs(ref))), np.max(np.abs(s2 - ref))
+    if case == "small":
+        assert np.all(np.abs(s2) < 1e-9)
+    le.close()
+
+
 def test_errors_are_reported():
     from paper_2209_04015_b200 import AfqmcError, LocalEnergy
     inp = make_inputs("tiny")
