@@ -27,6 +27,8 @@
  *     detected before any work is enqueued.
  *   - Tuning override (benchmarks only; results do not depend on it): the environment variable
  *     AFQMC_K2_PIPELINE="k,s" forces K2's shared-memory ring to s stages of k DMMA k-steps each when that fits.
+ *   - A handle owns one set of workspaces: calls on the same handle must be ordered (one stream, or streams the
+ *     caller has ordered with events); use one handle per concurrent stream.  Handles are independent of each other.
  *   - Requires compute capability 10.x (sm_100a); anything else returns AFQMC_ERR_ARCH.  There is no CPU path.
  */
 #ifndef AFQMC_H_

@@ -58,7 +58,8 @@ struct afqmc_ctx {
     double *e1 = nullptr, *logdet = nullptr;
     double2 *h_walkers = nullptr;      // device staging for the host-buffer entry point
     double *h_outE = nullptr, *h_outO = nullptr;
-    int last_nw = 0;
+    int last_nw = 0;                   // walkers whose theta the handle holds (last energy or force-bias-only call)
+    int last_energy_nw = 0;            // walkers whose Coulomb traces the handle holds (last energy call)
     bool fb_enabled = false;
     long long launches = 0;
     bool profiling = false;
@@ -101,24 +102,24 @@ size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages) {
     return nstages * stage + (size_t)strips * 4 * LD2 * 8 + (size_t)2 * K2_MAX_WT * K2_MAX_WM * 16 + (size_t)(2 * nstages + 2) * 8 + 16;
 }
 
-// Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer,
-// preferring the most k-steps in flight (capped at 12), then the larger chunk.
+// Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer.
 bool choose_pipeline(int strips, int NT, int ksteps, int &ksc, int &nst) {
     if (const char *ov = std::getenv("AFQMC_K2_PIPELINE")) {   // tuning override "ksc,stages" (include/afqmc.h)
         int kc = 0, s = 0;
-        if (std::sscanf(ov, "%d,%d", &kc, &s) == 2 && kc >= 1 && kc <= ksteps && s >= 3 && s <= 16 &&
+        if (std::sscanf(ov, "%d,%d", &kc, &s) == 2 && kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 &&
             k2_smem_bytes(strips, NT, kc, s) <= (size_t)kMaxSmem) {
             ksc = kc; nst = s;
             return true;
         }
     }
+    // Measured on cu2o2 (profiles/): with the non-blocking producer the most k-steps in flight
+    // wins, and at equal depth fewer, larger chunks win (5 x 2 stages 85.4 %, 3 x 3 84.8 %, 2 x 5 84.2 % of peak).
     int best = 0;
-    for (int kc = 4; kc >= 1; --kc) {
-        if (kc > ksteps) continue;
-        for (int s = 8; s >= 3; --s) {
+    for (int s = 2; s <= 5; ++s) {
+        for (int kc = std::min(12, std::max(2, ksteps / 10)); kc >= 1; --kc) {   // short K loops want short chunks (tile start-up)
+            if (kc > ksteps) continue;
             if (k2_smem_bytes(strips, NT, kc, s) > (size_t)kMaxSmem) continue;
-            const int inflight = std::min(kc * s, 12);
-            if (inflight > best) { best = inflight; ksc = kc; nst = s; }
+            if (kc * s > best) { best = kc * s; ksc = kc; nst = s; }
             break;
         }
     }
@@ -423,6 +424,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     ctx->launches += 1;
     if (ev) { CU_TRY(ctx, cudaEventRecord(ev[3], stream)); ctx->prof_calls += 1; }
     ctx->last_nw = n_walkers;
+    ctx->last_energy_nw = n_walkers;
     return AFQMC_OK;
 }
 
@@ -446,10 +448,10 @@ int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walk
 int afqmc_force_bias(afqmc_ctx *ctx, void *out, void *stream_) {
     if (!ctx) return AFQMC_ERR_ARG;
     if (!out) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias: null pointer argument");
-    if (ctx->last_nw < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias: no energy call has been made on this handle");
-    const long long total = (long long)ctx->last_nw * ctx->n_gamma * 2;
+    if (ctx->last_energy_nw < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias: no energy call has been made on this handle");
+    const long long total = (long long)ctx->last_energy_nw * ctx->n_gamma * 2;
     k3_force_bias<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream_>>>(
-        ctx->last_nw, ctx->n_gamma, ctx->sp[0].n, ctx->sp[1].n, ctx->sp[0].tbuf, ctx->sp[1].tbuf, reinterpret_cast<double *>(out));
+        ctx->last_energy_nw, ctx->n_gamma, ctx->sp[0].n, ctx->sp[1].n, ctx->sp[0].tbuf, ctx->sp[1].tbuf, reinterpret_cast<double *>(out));
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;
