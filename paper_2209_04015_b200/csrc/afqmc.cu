@@ -476,7 +476,7 @@ int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream_) {
         sc.f_n_ct_max = (maxw + sc.f_wT - 1) / sc.f_wT;
         // split K so that (row tiles x column tiles x K parts) fills whole rounds of the persistent grid
         const int ks_raw = (n * N + 3) / 4;
-        sc.f_ksc = std::min(4, ks_raw);
+        sc.f_ksc = std::min(12, ks_raw);
         int best_s = 1;
         double best_fill = 0.0;
         for (int sp = 1; sp <= 8; ++sp) {
@@ -490,7 +490,7 @@ int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream_) {
         sc.f_kps = ((ks_raw + best_s - 1) / best_s + sc.f_ksc - 1) / sc.f_ksc * sc.f_ksc;   // k-steps per part, whole chunks
         sc.f_ksteps = sc.f_kps * best_s;                                                   // padded with zero k-steps
         sc.f_nchunks = sc.f_kps / sc.f_ksc;
-        sc.f_nstages = 5;
+        sc.f_nstages = 2;
         sc.f_smem = (size_t)sc.f_nstages * sc.f_ksc * (sc.f_strips + sc.f_NT) * 256 + (size_t)2 * sc.f_nstages * 8 + 16;
         sc.f_layA = OperandLayout{1, sc.f_strips, sc.f_ksteps, sc.f_gT, (long long)sc.f_strips * sc.f_ksteps * 32};
         sc.f_layB = OperandLayout{1, sc.f_NT, sc.f_ksteps, sc.f_wT, (long long)sc.f_NT * sc.f_ksteps * 32};
