@@ -352,6 +352,22 @@ def main():
             del ow, oE, oO, oi
             torch.cuda.empty_cache()
 
+    # ---- baseline B: the paper's own half-rotated CPU algorithm (Listing 4) restated in numpy, same host cores ----
+    cpu_b = None
+    if cpu is not None:
+        from oracle.listing4_cpu import HalfRotated, local_energy_listing4
+        t0 = time.perf_counter()
+        hr = HalfRotated(inp.h1e, inp.chol, inp.psi_a, inp.psi_b)
+        t_setup = time.perf_counter() - t0
+        nb_w, t0 = 0, time.perf_counter()
+        while nb_w < inp.n_walkers and (nb_w < 2 or time.perf_counter() - t0 < 5.0):
+            local_energy_listing4(hr, inp.e0, inp.phi_a[nb_w], inp.phi_b[nb_w])
+            nb_w += 1
+        dt_b = time.perf_counter() - t0
+        cpu_b = {"value": nb_w / dt_b, "unit": UNIT, "cores": oracle_threads(), "kind": "paper_listing4_numpy",
+                 "sample": f"oracle/listing4_cpu.py on the first {nb_w} walkers ({dt_b:.1f} s; half-rotation setup "
+                           f"{t_setup:.1f} s not included, as on the GPU)"}
+
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -375,7 +391,8 @@ def main():
                                "tflops_incl_k1": flops_fb / (ms_fb * 1e-3) * 1e-12,
                                "speedup_vs_energy_step": (ms_total / args.steps) / ms_fb},
                 "roofline": roofline,
-                "cpu_baseline": cpu}
+                "cpu_baseline": cpu,
+                "cpu_baseline_listing4": cpu_b}
         if others is not None:
             line["other_configs"] = others
         print(json.dumps(line), flush=True)

@@ -267,3 +267,27 @@ def test_batch_front_end(tiny):
     E, lo = orc.local_energy_batch(inp, rung="O1", V=V)
     E3, lo3 = orc.local_energy_batch(inp, rung="O3", walkers=[1, 3])
     assert np.allclose(E3, E[[1, 3]], rtol=1e-12) and np.allclose(lo3, lo[[1, 3]], rtol=1e-12)
+
+
+@pytest.mark.parametrize("name,nw", [("tiny", 4), ("small", 3)])
+def test_listing4_agrees_with_definition(name, nw):
+    """The paper's own half-rotated CPU algorithm (oracle/listing4_cpu.py, baseline B) against the definition oracle."""
+    from oracle.listing4_cpu import HalfRotated, local_energy_listing4
+    inp = make_inputs(name, n_walkers=nw)
+    Eo, loo = orc.local_energy_batch(inp, rung="O1")
+    hr = HalfRotated(inp.h1e, inp.chol, inp.psi_a, inp.psi_b)
+    for w in range(nw):
+        E, lo = local_energy_listing4(hr, inp.e0, inp.phi_a[w], inp.phi_b[w])
+        assert rel(E, Eo[w]) < 1e-11
+        assert abs(lo.real - loo[w].real) < 1e-10 and abs(np.angle(np.exp(1j * (lo.imag - loo[w].imag)))) < 1e-10
+
+
+def test_listing4_complex_trial_unequal_spin():
+    from oracle.listing4_cpu import HalfRotated, local_energy_listing4
+    h1e, chol, e0, psi_a, psi_b, phis_a, phis_b = random_system(77, 9, 4, 2, 11, complex_trial=True)
+    V = orc.eri_from_cholesky(chol)
+    hr = HalfRotated(h1e, chol, psi_a, psi_b)
+    for w in range(len(phis_a)):
+        Eo = orc.local_energy_full_eri(h1e, V, e0, psi_a, psi_b, phis_a[w], phis_b[w])["E"]
+        E, _ = local_energy_listing4(hr, e0, phis_a[w], phis_b[w])
+        assert rel(E, Eo) < 1e-11
