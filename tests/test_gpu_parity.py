@@ -83,6 +83,18 @@ def test_parity_full_size_vs_golden(name):
     assert_parity(E[[w]], lo[[w]], Eo, loo)
 
 
+@pytest.mark.parametrize("name", ["medium", "cu2o2"])
+def test_parity_every_walker_full_size_vs_listing4(name):
+    """Every walker of the full-size launch (not only the sampled ones above) against the paper's half-rotated CPU
+    algorithm (oracle/listing4_cpu.py), which tests/test_oracle_pins.py pins to the definition oracle."""
+    from oracle.listing4_cpu import HalfRotated, local_energy_listing4
+    inp = make_inputs(name)
+    E, lo = gpu_energy(inp)
+    hr = HalfRotated(inp.h1e, inp.chol, inp.psi_a, inp.psi_b)
+    ref = [local_energy_listing4(hr, inp.e0, inp.phi_a[w], inp.phi_b[w]) for w in range(inp.n_walkers)]
+    assert_parity(E, lo, np.array([r[0] for r in ref]), np.array([r[1] for r in ref]))
+
+
 # ---- edge cases --------------------------------------------------------------------------------------
 def _custom(seed, N, na, nb, ng, nw, noise=0.2, complex_trial=False):
     rng = np.random.default_rng(seed)
