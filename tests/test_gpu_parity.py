@@ -204,6 +204,30 @@ def test_bitwise_determinism():
     le.close()
 
 
+def test_bitwise_determinism_full_size_and_mixed_batches():
+    """No compute-sanitizer on this pool, so races in K2's barrier protocol are hunted the slow way: the full-size
+    headline launch repeated, with batches of another size interleaved on the same handle, must reproduce bit for bit
+    (each batch shape against itself)."""
+    inp = make_inputs("cu2o2")
+    le = _le(inp)
+    w_all = torch.from_numpy(inp.walkers_packed()).cuda()
+    E0, lo0 = le.local_energy(w_all, inp.n_walkers)
+    E0, lo0 = E0.clone(), lo0.clone()
+    sub = [0, 17, 255, 128, 3]
+    w_sub = torch.from_numpy(inp.walkers_packed(sub)).cuda()
+    Es0 = None
+    for rep in range(6):
+        Es, _ = le.local_energy(w_sub, len(sub))
+        # another batch shape deals the (gamma, walker) blocks to the warps in another order: same walkers, other rounding
+        assert torch.all((Es - E0[sub]).abs() <= 1e-13 * E0[sub].abs()), rep
+        Es0 = Es.clone() if Es0 is None else Es0
+        assert torch.equal(Es.view(torch.float64), Es0.view(torch.float64)), rep
+        E1, lo1 = le.local_energy(w_all, inp.n_walkers)
+        assert torch.equal(E1.view(torch.float64), E0.view(torch.float64)), rep
+        assert torch.equal(lo1.view(torch.float64), lo0.view(torch.float64)), rep
+    le.close()
+
+
 def test_host_entry_point_and_force_bias():
     inp = make_inputs("small", n_walkers=6)
     le = _le(inp)
