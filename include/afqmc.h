@@ -126,6 +126,17 @@ int afqmc_force_bias_only(afqmc_ctx *ctx, const void *walkers, int n_walkers, vo
  */
 int afqmc_spin_squared(afqmc_ctx *ctx, void *out, void *stream);
 
+/*
+ * afqmc_greens_function -- optional full one-body Green's function of one spin sector, for user-written mixed
+ * estimators (the paper's greens_function(walkers, trial, build_full=True)):
+ *     G^sigma_pq = <psi_T|a+_p a_q|phi_w> / <psi_T|phi_w> = [phi S^-1 psi^dagger]_qp = sum_j theta^sigma_jq conj(psi^sigma_pj)
+ *                                                                                      PAPER.md:174, 187 (Eq. 20, 22)
+ * for the walkers of the most recent afqmc_local_energy / afqmc_force_bias_only call.
+ *   spin  0 = alpha, 1 = beta.   out: device, complex128 [n_walkers of that call][N][N], row-major in (p, q);
+ *   n_walkers * N * N * 16 bytes (344 MB per spin at N = 290, 256 walkers).  Enqueued on `stream`.
+ */
+int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream);
+
 /* Frees the handle and every internal buffer.  NULL is allowed. */
 void afqmc_destroy(afqmc_ctx *ctx);
 

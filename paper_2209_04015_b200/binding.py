@@ -14,7 +14,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias",
-           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_destroy",
+           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
            "afqmc_fp64_peak", "afqmc_plan"]
 
@@ -60,6 +60,8 @@ def load_library():
     lib.afqmc_force_bias_only.restype = ip
     lib.afqmc_spin_squared.argtypes = [vp, vp, vp]
     lib.afqmc_spin_squared.restype = ip
+    lib.afqmc_greens_function.argtypes = [vp, ip, vp, vp]
+    lib.afqmc_greens_function.restype = ip
     lib.afqmc_destroy.argtypes = [vp]
     lib.afqmc_destroy.restype = None
     lib.afqmc_last_error.argtypes = [vp]
@@ -209,6 +211,15 @@ class LocalEnergy:
         if out is None:
             out = torch.empty(n_walkers, dtype=torch.complex128, device="cuda")
         self._check(self._lib.afqmc_spin_squared(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_spin_squared")
+        return out
+
+    def greens_function(self, spin, n_walkers, out=None, stream=None):
+        """afqmc_greens_function: full G^sigma [n_walkers, N, N] complex128 (spin 0 = alpha, 1 = beta) for the walkers
+        of the last energy / force-bias call."""
+        if out is None:
+            out = torch.empty((n_walkers, self.N, self.N), dtype=torch.complex128, device="cuda")
+        self._check(self._lib.afqmc_greens_function(self._h, int(spin), out.data_ptr(), _stream_ptr(stream)),
+                    "afqmc_greens_function")
         return out
 
     def info(self) -> dict:

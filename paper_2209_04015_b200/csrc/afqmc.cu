@@ -20,6 +20,7 @@
 #include "k2_exchange.cuh"
 #include "k3_assemble.cuh"
 #include "k5_spin_squared.cuh"
+#include "k6_greens.cuh"
 
 using namespace afqmc;
 
@@ -574,6 +575,28 @@ int afqmc_spin_squared(afqmc_ctx *ctx, void *out, void *stream_) {
     const size_t smem = ((size_t)2 * na * nb + (size_t)2 * (na + nb) * K5_PCHUNK) * 16;
     CU_TRY(ctx, cudaFuncSetAttribute((const void *)k5_spin_squared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k5_spin_squared<<<ctx->last_nw, K5_THREADS, smem, (cudaStream_t)stream_>>>(p5);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!out || (spin != 0 && spin != 1)) return fail(ctx, AFQMC_ERR_ARG, "afqmc_greens_function: bad argument");
+    if (ctx->last_nw < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_greens_function: no energy or force-bias call has been made on this handle");
+    const SpinCfg &sc = ctx->sp[spin];
+    const int N = ctx->N;
+    if (sc.n == 0) {        // empty spin sector: G = 0
+        CU_TRY(ctx, cudaMemsetAsync(out, 0, (size_t)ctx->last_nw * N * N * 16, (cudaStream_t)stream_));
+        return AFQMC_OK;
+    }
+    K6Params p6{};
+    p6.N = N; p6.n = sc.n; p6.theta = sc.B; p6.layB = sc.layB; p6.psi = sc.psi; p6.psi_im = sc.psi_im;
+    p6.out = reinterpret_cast<double2 *>(out);
+    const size_t smem = (size_t)2 * sc.n * K6_TILE * 16;
+    CU_TRY(ctx, cudaFuncSetAttribute((const void *)k6_greens_function, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int nt = (N + K6_TILE - 1) / K6_TILE;
+    k6_greens_function<<<dim3(nt, nt, ctx->last_nw), 256, smem, (cudaStream_t)stream_>>>(p6);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;

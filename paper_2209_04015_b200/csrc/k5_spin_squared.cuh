@@ -1,7 +1,7 @@
 // K5 -- <S^2> mixed estimator for a single-determinant trial (Eq. 31; Listing 6):
 //   s2_w = N_dn + M_S (M_S + 1) - sum_pq G^up_pq G^dn_qp ,      M_S = (n_up - n_dn) / 2,
-// evaluated in half-rotated form (no N x N Green's function is built):  with G^s_pq = sum_j theta^s_jp conj(psi^s_qj)
-// (Eq. 22)
+// evaluated in half-rotated form (no N x N Green's function is built):  with G^s_pq = sum_j theta^s_jq conj(psi^s_pj)
+// (Eq. 22, matrix form)
 //   sum_pq G^up_pq G^dn_qp = sum_jk A_jk B_kj ,   A = theta^up conj(psi^dn)  (n_up x n_dn),   B = theta^dn conj(psi^up)  (n_dn x n_up).
 // theta is read from the packed planes K1 wrote for K2 (common.cuh).  One CTA per walker, fixed-order reduction.
 #pragma once

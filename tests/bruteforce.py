@@ -139,3 +139,26 @@ def brute_force_spin_squared(psi_a, psi_b, phi_a, phi_b):
                 np.add.at(bra, lookup[b4], a4)
     ms = 0.5 * (psi_a.shape[1] - psi_b.shape[1])
     return np.sum(np.conj(c_psi) * bra) / ovlp + ms * (ms + 1.0)
+
+
+def brute_force_greens_function(psi_a, psi_b, phi_a, phi_b, spin):
+    """G_pq = <psi|a+_{p,spin} a_{q,spin}|phi>/<psi|phi> (Eq. 20) by operator application on the
+    determinant expansion; spin 0 = alpha, 1 = beta.  Fixes the index ORDER of the Green's function, which the energy
+    (symmetric h and L) cannot see."""
+    N = psi_a.shape[0]
+    bits_phi, c_phi = _minor_expansion(phi_a, phi_b, N)
+    bits_psi, c_psi = _minor_expansion(psi_a, psi_b, N)
+    lookup = np.full(1 << (2 * N), -1, dtype=np.int64)
+    lookup[bits_psi] = np.arange(len(bits_psi))
+    phi_vec = np.zeros(len(bits_psi), dtype=np.complex128)
+    phi_vec[lookup[bits_phi]] = c_phi
+    ovlp = np.sum(np.conj(c_psi) * phi_vec)
+    off = spin * N
+    G = np.zeros((N, N), dtype=np.complex128)
+    for q in range(N):
+        b1, a1 = _annihilate(bits_phi, c_phi, off + q)
+        for p in range(N):
+            b2, a2 = _create(b1, a1, off + p)
+            if len(b2):
+                G[p, q] = np.sum(np.conj(c_psi[lookup[b2]]) * a2) / ovlp
+    return G

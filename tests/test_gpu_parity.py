@@ -302,6 +302,31 @@ def test_spin_squared_matches_oracle(case):
     le.close()
 
 
+@pytest.mark.parametrize("case", ["uhf", "complex", "one_spin", "n64"])
+def test_full_greens_function_matches_oracle(case):
+    """Optional full Green's function (Eq. 22; build_full=True of PAPER.md:412-414) against the oracle's
+    phi (psi^dagger phi)^-1 psi^dagger, and the paper's Listing 6 estimator evaluated from it against afqmc_spin_squared."""
+    inp = {"uhf": lambda: _custom(611, 33, 13, 11, 6, 4),
+           "complex": lambda: _custom(612, 21, 6, 5, 6, 3, complex_trial="both"),
+           "one_spin": lambda: _custom(613, 10, 4, 0, 5, 2),
+           "n64": lambda: _custom(614, 70, 64, 33, 4, 2)}[case]()
+    le = _le(inp)
+    gpu_energy(inp, le)
+    G = [le.greens_function(s, inp.n_walkers) for s in (0, 1)]
+    s2 = le.spin_squared(inp.n_walkers)
+    torch.cuda.synchronize()
+    for w in range(inp.n_walkers):
+        for s, (psi, phi) in enumerate(((inp.psi_a, inp.phi_a[w]), (inp.psi_b, inp.phi_b[w]))):
+            ref = orc.greens_function(psi, phi)[0]
+            got = G[s][w].cpu().numpy()
+            assert np.max(np.abs(got - ref)) <= 1e-10 * max(1.0, np.max(np.abs(ref))), (w, s)
+    # Listing 6 (PAPER.md:426): two_body = -einsum("zij,zji->z", Ga, Gb)
+    ms = 0.5 * (inp.n_alpha - inp.n_beta)
+    listing6 = inp.n_beta + ms * (ms + 1) - torch.einsum("zij,zji->z", G[0], G[1])
+    assert torch.all((listing6 - s2).abs() <= 1e-10 * torch.clamp(s2.abs(), min=1.0))
+    le.close()
+
+
 def test_errors_are_reported():
     from paper_2209_04015_b200 import AfqmcError, LocalEnergy
     inp = make_inputs("tiny")

@@ -291,3 +291,16 @@ def test_listing4_complex_trial_unequal_spin():
         Eo = orc.local_energy_full_eri(h1e, V, e0, psi_a, psi_b, phis_a[w], phis_b[w])["E"]
         E, _ = local_energy_listing4(hr, e0, phis_a[w], phis_b[w])
         assert rel(E, Eo) < 1e-11
+
+
+@pytest.mark.parametrize("complex_trial", [False, True])
+def test_greens_function_index_order_by_operator_application(complex_trial):
+    """G_pq = <a+_p a_q> (Eq. 20) element by element from the determinant expansion.  The energy cannot pin the index
+    order (h and L are symmetric), and Eq. 22's two members are transposes of each other (DESIGN.md section 3 #16)."""
+    from tests.bruteforce import brute_force_greens_function
+    h1e, chol, e0, psi_a, psi_b, phis_a, phis_b = random_system(91, 6, 3, 2, 2, complex_trial=complex_trial)
+    for spin, (psi, phi) in enumerate(((psi_a, phis_a[0]), (psi_b, phis_b[0]))):
+        G = orc.greens_function(psi, phi)[0]
+        ref = brute_force_greens_function(psi_a, psi_b, phis_a[0], phis_b[0], spin)
+        assert np.max(np.abs(G - ref)) < 1e-12
+        assert np.max(np.abs(G - G.T)) > 1e-3          # the case can tell G from its transpose
