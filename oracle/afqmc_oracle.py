@@ -330,3 +330,22 @@ def spin_squared(psi_a, psi_b, phi_a, phi_b):
     n_up, n_dn = psi_a.shape[1], psi_b.shape[1]
     ms = 0.5 * (n_up - n_dn)
     return n_dn + ms * (ms + 1.0) - np.einsum("ij,ji->", Ga, Gb)
+
+
+def phaseless_weight_update(weight, log_ovlp_old, log_ovlp_new, x, xbar):
+    """Phaseless weight update of one walker, PAPER.md:100-123 (Eq. 7, 8, 10-12), step by step in the paper's order:
+        O      = <Psi_T|B(x - xbar)|phi> / <Psi_T|phi>  = exp(log_ovlp_new - log_ovlp_old)               (Eq. 8)
+        I      = O * exp(x . xbar - xbar . xbar / 2)                                                      (Eq. 7)
+        theta  = arg O                                                                                    (Eq. 11)
+        I_ph   = |I| * max(0, cos theta)                                                                  (Eq. 10)
+        w_new  = I_ph * w                                                                                 (Eq. 12)
+    log-overlaps are (log|ovlp|, arg ovlp) as returned by the local-energy call for the walker before and after the
+    propagator was applied; x is the real auxiliary-field vector, xbar the complex force bias (Eq. 9).  The dot
+    products are plain (unconjugated) sums over the auxiliary index."""
+    x = np.asarray(x, dtype=np.float64)
+    xbar = np.asarray(xbar, dtype=np.complex128)
+    log_o = complex(log_ovlp_new) - complex(log_ovlp_old)
+    expo = np.sum(x * xbar) - 0.5 * np.sum(xbar * xbar)
+    big_i = np.exp(log_o + expo)
+    theta = math.atan2(math.sin(log_o.imag), math.cos(log_o.imag))      # arg O in (-pi, pi]
+    return abs(big_i) * max(0.0, math.cos(theta)) * weight
