@@ -137,6 +137,20 @@ int afqmc_spin_squared(afqmc_ctx *ctx, void *out, void *stream);
  */
 int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream);
 
+/*
+ * afqmc_phaseless_weights -- the weight update of the hybrid phaseless propagation (Eq. 7, 8, 10-12),
+ * for a caller that applies its own propagator B(x - xbar) to the walkers and evaluates the overlaps before and after
+ * with afqmc_local_energy / afqmc_force_bias_only:
+ *     O = exp(log_ovlp_new - log_ovlp_old),   I = O exp(x . xbar - xbar . xbar / 2),   w_new = |I| max(0, cos(arg O)) w
+ *   x             device, float64 [n_walkers][n_gamma]      auxiliary fields drawn by the caller (Eq. 4)
+ *   xbar          device, complex128 [n_walkers][n_gamma]   force bias (Eq. 9), e.g. from afqmc_force_bias_only
+ *   log_ovlp_old/new  device, complex128 [n_walkers]        (log|ovlp|, arg ovlp) as returned in out_overlaps
+ *   weights_in/out    device, float64 [n_walkers]           may alias
+ * No handle: the call keeps no state.  Enqueued on `stream`.
+ */
+int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const void *xbar, const void *log_ovlp_old,
+                            const void *log_ovlp_new, const double *weights_in, double *weights_out, void *stream);
+
 /* Frees the handle and every internal buffer.  NULL is allowed. */
 void afqmc_destroy(afqmc_ctx *ctx);
 

@@ -14,7 +14,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias",
-           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_destroy",
+           "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_phaseless_weights", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
            "afqmc_fp64_peak", "afqmc_plan"]
 
@@ -62,6 +62,8 @@ def load_library():
     lib.afqmc_spin_squared.restype = ip
     lib.afqmc_greens_function.argtypes = [vp, ip, vp, vp]
     lib.afqmc_greens_function.restype = ip
+    lib.afqmc_phaseless_weights.argtypes = [ip, ip, vp, vp, vp, vp, vp, vp, vp]
+    lib.afqmc_phaseless_weights.restype = ip
     lib.afqmc_destroy.argtypes = [vp]
     lib.afqmc_destroy.restype = None
     lib.afqmc_last_error.argtypes = [vp]
@@ -101,6 +103,27 @@ def fp64_peak_tflops(mode: str = "dmma", launches: int = 10) -> float:
     if rc != 0:
         raise AfqmcError(f"afqmc_fp64_peak failed ({rc}): {lib.afqmc_last_error(None).decode()}")
     return out.value
+
+
+def phaseless_weights(x, xbar, log_ovlp_old, log_ovlp_new, weights, out=None, stream=None):
+    """afqmc_phaseless_weights (Eq. 7-12): x float64 [Nw, Ngamma], xbar complex128 [Nw, Ngamma], log-overlaps
+    complex128 [Nw], weights float64 [Nw]; all contiguous CUDA tensors.  Returns the new weights."""
+    _require_cuda()
+    lib = load_library()
+    nw, ng = x.shape
+    for t, dt in ((x, torch.float64), (xbar, torch.complex128), (log_ovlp_old, torch.complex128),
+                  (log_ovlp_new, torch.complex128), (weights, torch.float64)):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise AfqmcError("phaseless_weights: inputs must be contiguous CUDA tensors of the documented dtypes")
+    if xbar.shape != x.shape or log_ovlp_old.numel() != nw or log_ovlp_new.numel() != nw or weights.numel() != nw:
+        raise AfqmcError("phaseless_weights: shapes do not match")
+    if out is None:
+        out = torch.empty_like(weights)
+    rc = lib.afqmc_phaseless_weights(nw, ng, x.data_ptr(), xbar.data_ptr(), log_ovlp_old.data_ptr(),
+                                     log_ovlp_new.data_ptr(), weights.data_ptr(), out.data_ptr(), _stream_ptr(stream))
+    if rc != 0:
+        raise AfqmcError(f"afqmc_phaseless_weights failed ({rc}): {lib.afqmc_last_error(None).decode()}")
+    return out
 
 
 def _info_dict(inf) -> dict:

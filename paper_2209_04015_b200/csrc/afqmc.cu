@@ -21,6 +21,7 @@
 #include "k3_assemble.cuh"
 #include "k5_spin_squared.cuh"
 #include "k6_greens.cuh"
+#include "k7_phaseless.cuh"
 
 using namespace afqmc;
 
@@ -599,6 +600,17 @@ int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream_) {
     k6_greens_function<<<dim3(nt, nt, ctx->last_nw), 256, smem, (cudaStream_t)stream_>>>(p6);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const void *xbar, const void *log_ovlp_old,
+                            const void *log_ovlp_new, const double *weights_in, double *weights_out, void *stream_) {
+    if (n_walkers < 1 || n_gamma < 1 || !x || !xbar || !log_ovlp_old || !log_ovlp_new || !weights_in || !weights_out)
+        return fail(nullptr, AFQMC_ERR_ARG, "afqmc_phaseless_weights: bad argument");
+    k7_phaseless_update<<<n_walkers, K7_THREADS, 0, (cudaStream_t)stream_>>>(
+        n_gamma, x, reinterpret_cast<const double *>(xbar), reinterpret_cast<const double *>(log_ovlp_old),
+        reinterpret_cast<const double *>(log_ovlp_new), weights_in, weights_out);
+    CU_TRY(nullptr, cudaGetLastError());
     return AFQMC_OK;
 }
 

@@ -327,6 +327,35 @@ def test_full_greens_function_matches_oracle(case):
     le.close()
 
 
+def test_phaseless_weight_update_matches_oracle():
+    """Eq. 7-12 on the GPU against the oracle, with real log-overlaps and force biases from the library (before / after
+    a made-up rotation of the walkers) and phases on both sides of the cos cut-off."""
+    from paper_2209_04015_b200 import phaseless_weights
+    inp = make_inputs("small", n_walkers=11, n_gamma=37)
+    le = _le(inp)
+    le.enable_force_bias(torch.from_numpy(inp.chol).cuda())
+    w0 = torch.from_numpy(inp.walkers_packed()).cuda()
+    xbar = le.force_bias_only(w0, 11).clone()
+    _, lo_old = le.local_energy(w0, 11)
+    lo_old = lo_old.clone()
+    rng = np.random.default_rng(5)
+    phase = np.exp(1j * np.linspace(-3.0, 3.0, 11))                 # rotates arg(ovlp) through the cut-off
+    phi_a2 = inp.phi_a * (1.0 + 0.05 * rng.standard_normal(inp.phi_a.shape)) * phase[:, None, None]
+    inp2 = Inputs(**{**inp.__dict__, "phi_a": np.ascontiguousarray(phi_a2)})
+    _, lo_new = le.local_energy(torch.from_numpy(inp2.walkers_packed()).cuda(), 11)
+    x = torch.from_numpy(rng.standard_normal((11, 37))).cuda()
+    xbar = (xbar * 1e-3).contiguous()                               # keep exp() in range for this synthetic Hamiltonian
+    wts = torch.from_numpy(rng.uniform(0.5, 2.0, 11)).cuda()
+    got = phaseless_weights(x, xbar, lo_old, lo_new, wts)
+    torch.cuda.synchronize()
+    ref = np.array([orc.phaseless_weight_update(wts[k].item(), complex(lo_old[k].item()), complex(lo_new[k].item()),
+                                                x[k].cpu().numpy(), xbar[k].cpu().numpy()) for k in range(11)])
+    got = got.cpu().numpy()
+    assert np.all(np.abs(got - ref) <= 1e-10 * np.maximum(np.abs(ref), 1e-300))
+    assert np.any(ref == 0.0) and np.any(ref > 0.0)
+    le.close()
+
+
 def test_errors_are_reported():
     from paper_2209_04015_b200 import AfqmcError, LocalEnergy
     inp = make_inputs("tiny")
