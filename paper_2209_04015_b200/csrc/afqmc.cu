@@ -470,6 +470,8 @@ int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream_) {
         const int n = sc.n;
         if (n == 0) continue;
         const int nbf = sc.cplx ? 2 : 1;                          // rows per gamma: Re (and Im) of Ltilde
+        cudaFree(sc.f_A); cudaFree(sc.f_B); cudaFree(sc.f_craw);  // a failed earlier attempt may have left some behind
+        sc.f_A = sc.f_B = sc.f_craw = nullptr;
         sc.f_wT = std::min(64, (maxw + 3) / 4 * 4);               // 2 * wT columns = 8 * NT
         sc.f_NT = sc.f_wT / 4;
         sc.f_strips = std::min(K2_MAX_WM, (n_gamma * nbf + 7) / 8);
@@ -698,8 +700,12 @@ int afqmc_fp64_peak(int mode, int launches, double *tflops, void *stream_) {
     if (int rc = check_arch(nullptr, &sms)) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
     double *d = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    struct Cleanup {                                   // releases the scratch on every return path
+        double *&d; cudaEvent_t &e0, &e1;
+        ~Cleanup() { if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); cudaFree(d); }
+    } cleanup{d, e0, e1};
     CU_TRY(nullptr, cudaMalloc(&d, 8));
-    cudaEvent_t e0, e1;
     CU_TRY(nullptr, cudaEventCreate(&e0));
     CU_TRY(nullptr, cudaEventCreate(&e1));
     const int iters = mode == 0 ? 20000 : 50000;
@@ -719,7 +725,6 @@ int afqmc_fp64_peak(int mode, int launches, double *tflops, void *stream_) {
     const double flops = mode == 0 ? 2.0 * 256 * PEAK_NACC * (double)iters * (threads / 32) * sms * launches
                                    : 2.0 * PEAK_NCH * (double)iters * threads * 2 * sms * launches;
     *tflops = flops / (ms * 1e-3) * 1e-12;
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     return AFQMC_OK;
 }
 
