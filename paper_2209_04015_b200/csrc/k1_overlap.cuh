@@ -14,6 +14,7 @@ namespace afqmc {
 
 constexpr int K1_THREADS = 256;
 constexpr int K1_PCHUNK = 32;  // rows of phi staged per pass = 8 DMMA k-steps of theta
+constexpr int K1_TU = 4;        // DMMA output tiles per warp and pass
 
 struct K1Params {
     const double2 *walkers;       // alpha block [Nw][N][na], then beta block [Nw][N][nb]
@@ -37,7 +38,7 @@ __device__ __forceinline__ double2 cmul(double2 a, double2 b) {
 }
 
 template <bool WITH_FB>
-__global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params P) {
+__global__ void __launch_bounds__(K1_THREADS, 4) k1_overlap_inverse_theta(K1Params P) {
     const int w = blockIdx.x, sp = blockIdx.y;
     const int n = P.n[sp], N = P.N;
     if (n == 0) return;
@@ -57,35 +58,56 @@ __global__ void __launch_bounds__(K1_THREADS) k1_overlap_inverse_theta(K1Params 
     const double *psi_im = P.psi_im[sp];
     const bool cplx = psi_im != nullptr;
 
-    // ---- S = psi^dagger phi = (Re psi - i Im psi)^T phi ------------------------------------------------------------------------
-    for (int e = tid; e < n * n; e += K1_THREADS) S[e] = make_double2(0.0, 0.0);
-    for (int p0 = 0; p0 < N; p0 += K1_PCHUNK) {
-        const int pc = min(K1_PCHUNK, N - p0);
-        __syncthreads();
-        for (int t = tid; t < pc * n; t += K1_THREADS) {
-            phis[t] = phi[(long long)p0 * n + t];
-            psis[t] = psi[(long long)p0 * n + t];
-            if (cplx) psii[t] = psi_im[(long long)p0 * n + t];
-        }
-        __syncthreads();
-        for (int e = tid; e < n * n; e += K1_THREADS) {
-            const int i = e / n, j = e - i * n;
-            double2 acc = S[e];
-            for (int pp = 0; pp < pc; ++pp) {
-                const double a = psis[pp * n + i];
-                const double2 f = phis[pp * n + j];
-                acc.x = fma(a, f.x, acc.x);
-                acc.y = fma(a, f.y, acc.y);
+    // ---- S = psi^dagger phi = (Re psi - i Im psi)^T phi  on the FP64 tensor cores ------------------------------------------
+    // Real TN product: rows i (8-row strips), columns (j, re/im) of the interleaved phi (8-column blocks), k = p.
+    // Warp `warp` owns the output tiles t = warp + 8 u; a tile's C fragment is exactly S[i][j] as (re, im) per lane.
+    const int ns = (n + 7) >> 3, ncb = (2 * n + 7) >> 3, ntile_s = ns * ncb;
+    // (K1_TU tiles per warp and pass; n <= 32 needs one pass, larger n re-streams phi once per pass)
+    for (int ubase = 0; ubase * 8 < ntile_s; ubase += K1_TU) {
+        double sacc[K1_TU][2];
+#pragma unroll
+        for (int u = 0; u < K1_TU; ++u) { sacc[u][0] = 0.0; sacc[u][1] = 0.0; }
+        const int fr = lane >> 2, fk = lane & 3;
+        const double *phid = reinterpret_cast<const double *>(phis);
+        for (int p0 = 0; p0 < N; p0 += K1_PCHUNK) {
+            const int pc = min(K1_PCHUNK, N - p0);
+            __syncthreads();
+            for (int t = tid; t < pc * n; t += K1_THREADS) {
+                phis[t] = phi[(long long)p0 * n + t];
+                psis[t] = psi[(long long)p0 * n + t];
+                if (cplx) psii[t] = psi_im[(long long)p0 * n + t];
             }
-            if (cplx) {
-                for (int pp = 0; pp < pc; ++pp) {
-                    const double b = psii[pp * n + i];
-                    const double2 f = phis[pp * n + j];
-                    acc.x = fma(b, f.y, acc.x);        // (a - ib)(fx + i fy) = (a fx + b fy) + i (a fy - b fx)
-                    acc.y = fma(-b, f.x, acc.y);
+            __syncthreads();
+#pragma unroll
+            for (int u = 0; u < K1_TU; ++u) {
+                const int t = warp + 8 * (ubase + u);
+                if (t < ntile_s) {
+                    const int st = t / ncb, cb = t - st * ncb;
+                    const int i = 8 * st + fr, col = 8 * cb + fr;               // A row / B column of this lane
+                    const bool iok = i < n, cok = col < 2 * n;
+                    for (int k0 = 0; k0 < pc; k0 += 4) {
+                        const int pp = k0 + fk;
+                        const bool pok = pp < pc;
+                        const double av = (iok && pok) ? psis[pp * n + i] : 0.0;
+                        const double bv = (cok && pok) ? phid[pp * 2 * n + col] : 0.0;
+                        dmma_m8n8k4(sacc[u][0], sacc[u][1], av, bv);
+                        if (cplx) {     // + Im psi^T (phi_im, -phi_re): (a - ib)(x + iy) = (ax + by) + i(ay - bx)
+                            const double av2 = (iok && pok) ? psii[pp * n + i] : 0.0;
+                            const double sw = (cok && pok) ? phid[pp * 2 * n + (col ^ 1)] : 0.0;
+                            dmma_m8n8k4(sacc[u][0], sacc[u][1], av2, (col & 1) ? -sw : sw);
+                        }
+                    }
                 }
             }
-            S[e] = acc;
+        }
+#pragma unroll
+        for (int u = 0; u < K1_TU; ++u) {
+            const int t = warp + 8 * (ubase + u);
+            if (t < ntile_s) {
+                const int st = t / ncb, cb = t - st * ncb;
+                const int i = 8 * st + fr, j = 4 * cb + fk;                     // C fragment: row lane/4, columns 2 (lane%4) + {0, 1}
+                if (i < n && j < n) S[i * n + j] = make_double2(sacc[u][0], sacc[u][1]);
+            }
         }
     }
     for (int e = tid; e < n; e += K1_THREADS) perm[e] = e;
