@@ -235,29 +235,43 @@ __global__ void __launch_bounds__(K1_THREADS, 4) k1_overlap_inverse_theta(K1Para
         const int pl = warp * 4 + kk;           // 8 warps x 4 = 32 rows of the chunk
         const int p = p0 + pl;
         if (p < Kpad) {
-            for (int j = jj; j < n; j += 8) {
-                double2 acc = make_double2(0.0, 0.0);
+            // two columns j, j + 8 per pass share every phi element fetched (same i order per sum as one column at a time)
+            for (int jb = jj; jb < n; jb += 16) {
+                double2 acc[2];
+#pragma unroll
+                for (int t = 0; t < 2; ++t) acc[t] = make_double2(0.0, 0.0);
+                const bool j1ok = jb + 8 < n;
                 if (p < N) {
                     const double2 *fr = phis + pl * n;
+                    const int j1 = j1ok ? jb + 8 : jb;
                     for (int i = 0; i < n; ++i) {
-                        const double2 f = fr[i], x = X[i * n + j];
-                        acc.x = fma(f.x, x.x, acc.x); acc.x = fma(-f.y, x.y, acc.x);
-                        acc.y = fma(f.x, x.y, acc.y); acc.y = fma(f.y, x.x, acc.y);
-                    }
-                    const double hv = ht[(long long)j * N + p];
-                    e1r = fma(hv, acc.x, e1r);
-                    e1i = fma(hv, acc.y, e1i);
-                    if (cplx) {
-                        const double hi = ht_im[(long long)j * N + p];
-                        e1r = fma(-hi, acc.y, e1r);
-                        e1i = fma(hi, acc.x, e1i);
+                        const double2 f = fr[i], x0 = X[i * n + jb], x1 = X[i * n + j1];
+                        acc[0].x = fma(f.x, x0.x, acc[0].x); acc[0].x = fma(-f.y, x0.y, acc[0].x);
+                        acc[0].y = fma(f.x, x0.y, acc[0].y); acc[0].y = fma(f.y, x0.x, acc[0].y);
+                        acc[1].x = fma(f.x, x1.x, acc[1].x); acc[1].x = fma(-f.y, x1.y, acc[1].x);
+                        acc[1].y = fma(f.x, x1.y, acc[1].y); acc[1].y = fma(f.y, x1.x, acc[1].y);
                     }
                 }
-                out[packed_offset(lay, tile, col_re + j, p)] = acc.x;
-                out[packed_offset(lay, tile, col_im + j, p)] = acc.y;
-                if (WITH_FB && p < N) {
-                    outF[packed_offset(layF, tileF, wlF, j * N + p)] = acc.x;
-                    outF[packed_offset(layF, tileF, layF.per_tile + wlF, j * N + p)] = acc.y;
+#pragma unroll
+                for (int t = 0; t < 2; ++t) {
+                    const int j = jb + 8 * t;
+                    if (t == 1 && !j1ok) continue;
+                    if (p < N) {
+                        const double hv = ht[(long long)j * N + p];
+                        e1r = fma(hv, acc[t].x, e1r);
+                        e1i = fma(hv, acc[t].y, e1i);
+                        if (cplx) {
+                            const double hi = ht_im[(long long)j * N + p];
+                            e1r = fma(-hi, acc[t].y, e1r);
+                            e1i = fma(hi, acc[t].x, e1i);
+                        }
+                    }
+                    out[packed_offset(lay, tile, col_re + j, p)] = acc[t].x;
+                    out[packed_offset(lay, tile, col_im + j, p)] = acc[t].y;
+                    if (WITH_FB && p < N) {
+                        outF[packed_offset(layF, tileF, wlF, j * N + p)] = acc[t].x;
+                        outF[packed_offset(layF, tileF, layF.per_tile + wlF, j * N + p)] = acc[t].y;
+                    }
                 }
             }
         }
