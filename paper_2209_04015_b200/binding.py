@@ -165,6 +165,8 @@ class LocalEnergy:
         if rc != 0:
             raise AfqmcError(f"afqmc_create failed ({rc}): {self._lib.afqmc_last_error(None).decode()}")
         self.N, self.n_alpha, self.n_beta, self.n_gamma, self.max_walkers = N, n_alpha, n_beta, n_gamma, max_walkers
+        self._last_nw = 0           # walkers of the last local_energy / force_bias_only call (theta held by the handle)
+        self._last_energy_nw = 0    # walkers of the last local_energy call (Coulomb traces held by the handle)
 
     def _check(self, rc, what):
         if rc != 0:
@@ -183,6 +185,7 @@ class LocalEnergy:
         rc = self._lib.afqmc_local_energy(self._h, walkers.data_ptr(), n_walkers, out_energies.data_ptr(),
                                           out_overlaps.data_ptr(), _stream_ptr(stream))
         self._check(rc, "afqmc_local_energy")
+        self._last_nw = self._last_energy_nw = n_walkers
         return out_energies, out_overlaps
 
     def local_energy_host(self, walkers_host, n_walkers, out_energies_host=None, out_overlaps_host=None, stream=None):
@@ -199,12 +202,27 @@ class LocalEnergy:
                                                out_energies_host.data_ptr(), out_overlaps_host.data_ptr(),
                                                _stream_ptr(stream))
         self._check(rc, "afqmc_local_energy_host")
+        self._last_nw = self._last_energy_nw = n_walkers
         return out_energies_host, out_overlaps_host
 
-    def force_bias(self, n_walkers, out=None, stream=None):
-        """afqmc_force_bias: [n_walkers, n_gamma] complex128 traces of the last energy call."""
+    def _out_for_last_call(self, what, n_walkers, last, per_walker, out):
+        """The library writes results for the walkers of the LAST call, not for a caller-chosen count: the optional
+        ``n_walkers`` must agree with it and a caller-provided ``out`` must hold exactly that many."""
+        if last < 1:
+            raise AfqmcError(f"{what}: no preceding energy / force-bias call on this handle")
+        if n_walkers is not None and n_walkers != last:
+            raise AfqmcError(f"{what}: n_walkers={n_walkers} but the handle holds {last} walkers from the last call")
+        shape = (last, *per_walker)
         if out is None:
-            out = torch.empty((n_walkers, self.n_gamma), dtype=torch.complex128, device="cuda")
+            return torch.empty(shape, dtype=torch.complex128, device="cuda")
+        if not (out.is_cuda and out.is_contiguous() and out.dtype == torch.complex128) or out.numel() != \
+                torch.Size(shape).numel():
+            raise AfqmcError(f"{what}: out must be a contiguous CUDA complex128 tensor of shape {shape}")
+        return out
+
+    def force_bias(self, n_walkers=None, out=None, stream=None):
+        """afqmc_force_bias: [n_walkers, n_gamma] complex128 traces of the last energy call."""
+        out = self._out_for_last_call("force_bias", n_walkers, self._last_energy_nw, (self.n_gamma,), out)
         self._check(self._lib.afqmc_force_bias(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_force_bias")
         return out
 
@@ -224,23 +242,25 @@ class LocalEnergy:
             raise AfqmcError("walkers has the wrong number of elements")
         if out is None:
             out = torch.empty((n_walkers, self.n_gamma), dtype=torch.complex128, device=walkers.device)
+        elif not (out.is_cuda and out.is_contiguous() and out.dtype == torch.complex128) or \
+                out.numel() != n_walkers * self.n_gamma:
+            raise AfqmcError("force_bias_only: out must be a contiguous CUDA complex128 [n_walkers, n_gamma] tensor")
         self._check(self._lib.afqmc_force_bias_only(self._h, walkers.data_ptr(), n_walkers, out.data_ptr(),
                                                     _stream_ptr(stream)), "afqmc_force_bias_only")
+        self._last_nw = n_walkers
         return out
 
-    def spin_squared(self, n_walkers, out=None, stream=None):
+    def spin_squared(self, n_walkers=None, out=None, stream=None):
         """afqmc_spin_squared: [n_walkers] complex128 <S^2> mixed estimator for the walkers of the last energy /
         force-bias call."""
-        if out is None:
-            out = torch.empty(n_walkers, dtype=torch.complex128, device="cuda")
+        out = self._out_for_last_call("spin_squared", n_walkers, self._last_nw, (), out)
         self._check(self._lib.afqmc_spin_squared(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_spin_squared")
         return out
 
-    def greens_function(self, spin, n_walkers, out=None, stream=None):
+    def greens_function(self, spin, n_walkers=None, out=None, stream=None):
         """afqmc_greens_function: full G^sigma [n_walkers, N, N] complex128 (spin 0 = alpha, 1 = beta) for the walkers
         of the last energy / force-bias call."""
-        if out is None:
-            out = torch.empty((n_walkers, self.N, self.N), dtype=torch.complex128, device="cuda")
+        out = self._out_for_last_call("greens_function", n_walkers, self._last_nw, (self.N, self.N), out)
         self._check(self._lib.afqmc_greens_function(self._h, int(spin), out.data_ptr(), _stream_ptr(stream)),
                     "afqmc_greens_function")
         return out

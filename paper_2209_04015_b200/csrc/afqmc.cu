@@ -51,6 +51,17 @@ struct SpinCfg {
 
 thread_local std::string g_create_error;
 
+// Tuning override AFQMC_K2_PIPELINE="ksc,stages" (include/afqmc.h), read once per process.
+struct PipelineOverride { bool set = false; int ksc = 0, stages = 0; };
+const PipelineOverride &pipeline_override() {
+    static const PipelineOverride ov = [] {
+        PipelineOverride o;
+        if (const char *e = std::getenv("AFQMC_K2_PIPELINE")) o.set = std::sscanf(e, "%d,%d", &o.ksc, &o.stages) == 2;
+        return o;
+    }();
+    return ov;
+}
+
 }  // namespace
 
 struct afqmc_ctx {
@@ -106,10 +117,9 @@ size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages) {
 
 // Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer.
 bool choose_pipeline(int strips, int NT, int ksteps, int &ksc, int &nst) {
-    if (const char *ov = std::getenv("AFQMC_K2_PIPELINE")) {   // tuning override "ksc,stages" (include/afqmc.h)
-        int kc = 0, s = 0;
-        if (std::sscanf(ov, "%d,%d", &kc, &s) == 2 && kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 &&
-            k2_smem_bytes(strips, NT, kc, s) <= (size_t)kMaxSmem) {
+    if (const PipelineOverride &ov = pipeline_override(); ov.set) {
+        const int kc = ov.ksc, s = ov.stages;
+        if (kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 && k2_smem_bytes(strips, NT, kc, s) <= (size_t)kMaxSmem) {
             ksc = kc; nst = s;
             return true;
         }
@@ -230,6 +240,17 @@ void free_ctx(afqmc_ctx *c) {
     delete c;
 }
 
+// Opt a kernel in to the full 227 KB of dynamic shared memory.  The attribute is process-global per kernel, so it is
+// always set to the ceiling: a smaller per-handle value would lower the cap for another spin or handle that shares
+// the instantiation (the launch itself passes the exact size).
+template <class Fn>
+cudaError_t allow_max_smem(Fn fn) {
+    cudaFuncAttributes fa{};
+    if (cudaError_t e = cudaFuncGetAttributes(&fa, (const void *)fn); e != cudaSuccess) return e;
+    return cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                kMaxSmem - (int)fa.sharedSizeBytes);   // static + dynamic <= 227 KB
+}
+
 int check_arch(afqmc_ctx *ctx, int *num_sms) {
     int dev = 0;
     CU_TRY(ctx, cudaGetDevice(&dev));
@@ -340,7 +361,7 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         CR_TRY(cudaMemsetAsync(sc.A, 0, sc.A_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.B, 0, sc.B_bytes, stream));
         CR_TRY(cudaMemsetAsync(sc.tbuf, 0, (size_t)max_walkers * n_gamma * 16, stream));
-        dim3 grid((N + 127) / 128, n_gamma);
+        dim3 grid(n_gamma, (N + 127) / 128);
         k0_half_rotate_h<<<(n * N + 255) / 256, 256, 0, stream>>>(h1e, sc.psi, N, n, 1.0, sc.ht);
         CR_TRY(cudaGetLastError());
         k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, sc.nb, 0, 1.0, sc.layA, sc.A, OperandLayout{}, nullptr);
@@ -358,11 +379,12 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
             free_ctx(c);
             return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: no K2 instantiation for MT=%d NT=%d", sc.MT, sc.NT);
         }
-        CR_TRY(cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc.k2_smem));
+        CR_TRY(allow_max_smem(fn));
     }
-    size_t k1s = std::max(c->sp[0].k1_smem, c->sp[1].k1_smem);
-    CR_TRY(cudaFuncSetAttribute((const void *)k1_overlap_inverse_theta<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k1s));
-    CR_TRY(cudaFuncSetAttribute((const void *)k1_overlap_inverse_theta<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k1s));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<false>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<true>));
+    CR_TRY(allow_max_smem(k5_spin_squared));
+    CR_TRY(allow_max_smem(k6_greens_function));
     CR_TRY(cudaMalloc(&c->e1, (size_t)2 * max_walkers * 16));
     CR_TRY(cudaMalloc(&c->logdet, (size_t)2 * max_walkers * 16));
     CR_TRY(cudaMemsetAsync(c->e1, 0, (size_t)2 * max_walkers * 16, stream));
@@ -505,7 +527,7 @@ int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream_) {
         CU_TRY(ctx, cudaMalloc(&sc.f_craw, c_bytes));
         CU_TRY(ctx, cudaMemsetAsync(sc.f_A, 0, a_bytes, stream));
         CU_TRY(ctx, cudaMemsetAsync(sc.f_B, 0, b_bytes, stream));
-        dim3 grid((N + 127) / 128, n_gamma);
+        dim3 grid(n_gamma, (N + 127) / 128);
         k0_half_rotate_chol<<<grid, 128, 0, stream>>>(chol, sc.psi, N, n, n_gamma, n * nbf, 0, 1.0, OperandLayout{}, nullptr, sc.f_layA, sc.f_A);
         CU_TRY(ctx, cudaGetLastError());
         ctx->launches += 1;
@@ -516,7 +538,7 @@ int afqmc_enable_force_bias(afqmc_ctx *ctx, const double *chol, void *stream_) {
         }
         K2FbFn fn = k2_pick_fb(sc.f_NT);
         if (!fn) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_enable_force_bias: no kernel for NT=%d", sc.f_NT);
-        CU_TRY(ctx, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc.f_smem));
+        CU_TRY(ctx, allow_max_smem(fn));
     }
     CU_TRY(ctx, cudaStreamSynchronize(stream));
     ctx->fb_enabled = true;
@@ -576,7 +598,6 @@ int afqmc_spin_squared(afqmc_ctx *ctx, void *out, void *stream_) {
     }
     const int na = p5.n[0], nb = p5.n[1];
     const size_t smem = ((size_t)2 * na * nb + (size_t)2 * (na + nb) * K5_PCHUNK) * 16;
-    CU_TRY(ctx, cudaFuncSetAttribute((const void *)k5_spin_squared, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k5_spin_squared<<<ctx->last_nw, K5_THREADS, smem, (cudaStream_t)stream_>>>(p5);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
@@ -597,9 +618,8 @@ int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream_) {
     p6.N = N; p6.n = sc.n; p6.theta = sc.B; p6.layB = sc.layB; p6.psi = sc.psi; p6.psi_im = sc.psi_im;
     p6.out = reinterpret_cast<double2 *>(out);
     const size_t smem = (size_t)2 * sc.n * K6_TILE * 16;
-    CU_TRY(ctx, cudaFuncSetAttribute((const void *)k6_greens_function, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int nt = (N + K6_TILE - 1) / K6_TILE;
-    k6_greens_function<<<dim3(nt, nt, ctx->last_nw), 256, smem, (cudaStream_t)stream_>>>(p6);
+    k6_greens_function<<<dim3(ctx->last_nw, nt, nt), 256, smem, (cudaStream_t)stream_>>>(p6);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;

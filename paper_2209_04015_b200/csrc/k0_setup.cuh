@@ -20,7 +20,7 @@ __global__ void k0_half_rotate_h(const double *__restrict__ h1e, const double *_
     ht[idx] = scale * acc;
 }
 
-// Ltilde: grid = (ceil(N/128), n_gamma); thread owns one (gamma, r) and produces all i in blocks of 8.
+// Ltilde: grid = (n_gamma, ceil(N/128)); thread owns one (gamma, r) and produces all i in blocks of 8.
 // psi is staged in shared memory by (p-chunk, 8 columns).
 constexpr int K0_PCHUNK = 64;
 
@@ -32,11 +32,11 @@ k0_half_rotate_chol(const double *__restrict__ chol, const double *__restrict__ 
     // packedF (may be null): the force-bias operand, rows (gamma[, part]), k = i * N + p   (Eq. 24).
     const int nbf = rows_per_gamma / n, part = row_shift / n;
     __shared__ double psi_s[K0_PCHUNK * 8];  // [K0_PCHUNK][8]
-    const int g = blockIdx.y;
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int g = blockIdx.x;                                  // gamma on grid.x: no 65535 limit
+    const int r = blockIdx.y * blockDim.x + threadIdx.x;
     const double *Lg = chol + (size_t)g * N * N;
-    const int tile = g / lay.per_tile;
-    const int row0 = (g - tile * lay.per_tile) * rows_per_gamma + row_shift;
+    const int tile = packedA ? g / lay.per_tile : 0;           // `lay` is empty when only packedF is wanted
+    const int row0 = packedA ? (g - tile * lay.per_tile) * rows_per_gamma + row_shift : 0;
     for (int i0 = 0; i0 < n; i0 += 8) {
         double acc[8];
 #pragma unroll

@@ -3,7 +3,7 @@
 //   G^sigma_pq = [phi (psi^dagger phi)^-1 psi^dagger]_qp = sum_j theta^sigma_jq conj(psi^sigma_pj)     PAPER.md:187 (Eq. 22, the
 //   matrix form; its last member, sum_j theta_jp (psi^dagger)_jq, is the transpose of it -- DESIGN.md section 3 #16)
 // from the theta planes K1 left in the handle (packed B operand, common.cuh).  Output [Nw][N][N] complex128, row-major
-// in (p, q).  Grid (ceil(N/32), ceil(N/32), Nw), 256 threads: a 32 x 32 tile of G per CTA, 4 elements per thread.
+// in (p, q).  Grid (Nw, ceil(N/32), ceil(N/32)), 256 threads: a 32 x 32 tile of G per CTA, 4 elements per thread.
 #pragma once
 #include "common.cuh"
 
@@ -21,8 +21,8 @@ struct K6Params {
 
 __global__ void __launch_bounds__(256) k6_greens_function(K6Params P) {
     extern __shared__ __align__(16) unsigned char k6_smem[];
-    const int n = P.n, N = P.N, w = blockIdx.z;
-    const int p0 = blockIdx.x * K6_TILE, q0 = blockIdx.y * K6_TILE;
+    const int n = P.n, N = P.N, w = blockIdx.x;               // walker on grid.x: no 65535 limit
+    const int p0 = blockIdx.y * K6_TILE, q0 = blockIdx.z * K6_TILE;
     double2 *th = reinterpret_cast<double2 *>(k6_smem);       // [n][32]  theta_jq for the tile's q
     double2 *ps = th + n * K6_TILE;                           // [n][32]  conj(psi_pj) for the tile's p
     const OperandLayout lay = P.layB;

@@ -30,7 +30,11 @@ PLAN = {
     "small": ("O1", "all", "all"),
     "medium": ("O2", [0, 1, 2, 63, 64, 126, 127], list(range(0, 128, 8)) + [1, 2, 63, 126, 127]),
     "cu2o2": ("O2", [0, 1, 127, 128, 254, 255], list(range(0, 256, 16)) + [1, 127, 254, 255]),
-    "large": (None, [], [0, 1, 255, 256, 510, 511]),
+    # large runs K2 with one walker per column tile (wT = 1) and is the only config on the <2,13> kernel with a 6 x 2
+    # ring: first / last walkers, both sides of the 148-CTA round boundaries of the tile schedule (147|148, 295|296,
+    # 443|444), both sides of the power-of-two marks and a few in between.
+    "large": (None, [], [0, 1, 2, 63, 64, 127, 128, 147, 148, 191, 192, 255, 256, 295, 296, 319, 320, 383, 384, 443, 444,
+                         447, 448, 477, 500, 509, 510, 511, 37, 101, 222, 350, 413, 470]),
 }
 
 

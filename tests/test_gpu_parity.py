@@ -159,6 +159,67 @@ def test_parity_complex_trial(N, na, nb, ng, nw, which):
     le.close()
 
 
+def test_unequal_spins_sharing_one_kernel_instantiation():
+    """Both spins map to the same K2 template instance with different shared-memory sizes (the opt-in
+    attribute is process-global per instantiation, so the smaller spin must not lower the cap for the larger)."""
+    from paper_2209_04015_b200 import plan
+    p = plan(50, 19, 15, 7, 1)
+    assert (p["mt"][0], p["nt"][0]) == (p["mt"][1], p["nt"][1]) and p["k2_smem_bytes"][0] != p["k2_smem_bytes"][1]
+    inp = _custom(901, 50, 19, 15, 7, 1)
+    Eo, loo = orc.local_energy_batch(inp, rung="O3")
+    E, lo = gpu_energy(inp)
+    assert_parity(E, lo, Eo, loo)
+
+
+def test_two_live_handles_of_different_size_used_alternately():
+    """Handles are independent (include/afqmc.h): a second, smaller handle created while the first is alive must not
+    disturb the first one's launches (shared-memory opt-in, workspaces), and vice versa."""
+    big = make_inputs("small", n_walkers=9)
+    small = _custom(902, 12, 5, 2, 9, 3)
+    le_big = _le(big)
+    E_big0, lo_big0 = gpu_energy(big, le_big)
+    le_small = _le(small)
+    Eo_s, loo_s = orc.local_energy_batch(small, rung="O1")
+    Eo_b, loo_b = orc.local_energy_batch(big, rung="O3")
+    for _ in range(2):
+        E_s, lo_s = gpu_energy(small, le_small)
+        assert_parity(E_s, lo_s, Eo_s, loo_s)
+        E_b, lo_b = gpu_energy(big, le_big)
+        assert_parity(E_b, lo_b, Eo_b, loo_b)
+        assert np.array_equal(E_b.view(np.float64), E_big0.view(np.float64))
+    le_big.enable_force_bias(torch.from_numpy(big.chol).cuda())
+    le_small.enable_force_bias(torch.from_numpy(small.chol).cuda())
+    fb_b = le_big.force_bias_only(torch.from_numpy(big.walkers_packed()).cuda(), 9)
+    fb_s = le_small.force_bias_only(torch.from_numpy(small.walkers_packed()).cuda(), 3)
+    fb_b2 = le_big.force_bias_only(torch.from_numpy(big.walkers_packed()).cuda(), 9)
+    torch.cuda.synchronize()
+    assert torch.equal(fb_b.view(torch.float64), fb_b2.view(torch.float64))
+    ref = orc.force_bias(small.chol, small.psi_a, small.psi_b, small.phi_a[1], small.phi_b[1])
+    assert np.all(np.abs(fb_s.cpu().numpy()[1] - ref) <= 1e-10 * np.max(np.abs(ref)))
+    le_big.close()
+    le_small.close()
+
+
+def test_outputs_of_the_last_call_are_sized_by_the_library_not_the_caller():
+    """force_bias / spin_squared / greens_function write results for the walkers of the LAST call; the
+    binding sizes `out` from that and rejects a caller-supplied count or buffer that disagrees."""
+    from paper_2209_04015_b200 import AfqmcError
+    inp = make_inputs("tiny")
+    le = _le(inp)
+    with pytest.raises(AfqmcError, match="no preceding"):
+        le.spin_squared()
+    gpu_energy(inp, le)
+    assert le.force_bias().shape == (4, inp.n_gamma) and le.spin_squared().shape == (4,)
+    assert le.greens_function(1).shape == (4, inp.N, inp.N)
+    with pytest.raises(AfqmcError, match="holds 4 walkers"):
+        le.force_bias(2)
+    with pytest.raises(AfqmcError, match="shape"):
+        le.greens_function(0, out=torch.empty((2, inp.N, inp.N), dtype=torch.complex128, device="cuda"))
+    gpu_energy(inp, le, [1, 3])
+    assert le.spin_squared().shape == (2,)
+    le.close()
+
+
 def test_fewer_walkers_than_capacity_and_ragged_tail():
     inp = make_inputs("small", n_walkers=13)
     le = _le(inp, max_walkers=64)
