@@ -60,7 +60,8 @@ enum {
  *          occupied orbitals; orthonormal columns expected).  A spin block whose imaginary part is
  *          identically zero (all of BASELINE.json's configs) takes the real-Ltilde path of PAPER.md:212 (two real
  *          products per complex T); a block with a non-zero imaginary part takes the four-product path (Ltilde
- *          stored as stacked Re / Im rows), at twice the arithmetic.  Non-finite entries return AFQMC_ERR_ARG.
+ *          stored as stacked Re / Im rows), at twice the arithmetic; such a block supports n_sigma <= 52 (2 n_sigma
+ *          rows must fit one K2 tile), beyond that AFQMC_ERR_UNSUPPORTED.  Non-finite entries return AFQMC_ERR_ARG.
  *   N >= 1; 0 <= n_alpha, n_beta <= min(N, AFQMC_MAX_NOCC); n_alpha + n_beta >= 1; n_gamma >= 1.
  *   e0     constant energy E0 added to every walker's energy.
  *   max_walkers >= 1 sizes the internal workspaces (theta, partial sums).
@@ -180,6 +181,10 @@ int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info);
  * operand sizes afqmc_create would choose for these sizes (kernel_launches = 0).  Same argument checks and
  * error codes as afqmc_create. */
 int afqmc_plan(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, afqmc_info *info);
+/* afqmc_plan_trial -- the same for a trial whose alpha / beta block is complex (complex_alpha / complex_beta != 0:
+ * the four-product path, 2 n_sigma rows per gamma block); afqmc_plan is the all-real case. */
+int afqmc_plan_trial(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, int complex_alpha, int complex_beta,
+                     afqmc_info *info);
 
 /* Per-kernel device times of energy calls.  enable != 0 makes every later afqmc_local_energy record CUDA
  * events around K1, K2 (both spins) and K3 on the caller's stream. */

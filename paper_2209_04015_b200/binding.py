@@ -16,7 +16,7 @@ _LIB = None
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias",
            "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_phaseless_weights", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
-           "afqmc_fp64_peak", "afqmc_plan"]
+           "afqmc_fp64_peak", "afqmc_plan", "afqmc_plan_trial"]
 
 
 class AfqmcError(RuntimeError):
@@ -80,6 +80,8 @@ def load_library():
     lib.afqmc_fp64_peak.restype = ip
     lib.afqmc_plan.argtypes = [ip, ip, ip, ip, ip, C.POINTER(AfqmcInfo)]
     lib.afqmc_plan.restype = ip
+    lib.afqmc_plan_trial.argtypes = [ip, ip, ip, ip, ip, ip, ip, C.POINTER(AfqmcInfo)]
+    lib.afqmc_plan_trial.restype = ip
     _LIB = lib
     return lib
 
@@ -134,11 +136,13 @@ def _info_dict(inf) -> dict:
     return out
 
 
-def plan(N, n_alpha, n_beta, n_gamma, max_walkers) -> dict:
-    """afqmc_plan: the K2 tile shape / pipeline / packed sizes afqmc_create would choose (host only, no GPU)."""
+def plan(N, n_alpha, n_beta, n_gamma, max_walkers, complex_alpha=False, complex_beta=False) -> dict:
+    """afqmc_plan / afqmc_plan_trial: the K2 tile shape / pipeline / packed sizes afqmc_create would choose (host only,
+    no GPU); complex_* say which spin blocks of the trial are complex."""
     lib = load_library()
     inf = AfqmcInfo()
-    rc = lib.afqmc_plan(N, n_alpha, n_beta, n_gamma, max_walkers, C.byref(inf))
+    rc = lib.afqmc_plan_trial(N, n_alpha, n_beta, n_gamma, max_walkers, int(bool(complex_alpha)),
+                              int(bool(complex_beta)), C.byref(inf))
     if rc != 0:
         raise AfqmcError(f"afqmc_plan failed ({rc}): {lib.afqmc_last_error(None).decode()}")
     return _info_dict(inf)

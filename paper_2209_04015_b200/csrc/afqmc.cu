@@ -147,33 +147,31 @@ bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
     if (n == 0) return true;
     const int ksteps = (N + 3) / 4;
     double best = -1.0;
-    const int wms[3] = {12, 8, 4};
-    const double wf[3] = {1.0, 0.97, 0.85};   // measured DMMA+LDS efficiency vs resident warps (profiles/fp64_peak_r1.md)
+    // Every warp of the CTA is an MMA warp: K2_MAX_WM = 12 warps (3 per SM sub-partition) is what the register file
+    // allows at 168 registers per thread, and fewer warps never scored higher in any shape.
+    const int WM = K2_MAX_WM;
     for (int wT = 1; wT <= K2_MAX_WT; ++wT) {
         const int cols = 2 * wT * n, NT = (cols + 7) / 8;
         if (NT > 16) continue;
         const double colEff = cols / (8.0 * NT);
-        for (int wi = 0; wi < 3; ++wi) {
-            const int WM = wms[wi];
-            for (int MT = 1; MT <= 4; ++MT) {
-                if (MT * NT > kMaxAcc) continue;
-                for (int gT = 1; gT <= n_gamma; ++gT) {
-                    const int strips = (gT * nb + 7) / 8;
-                    if (strips > MT * WM) break;
-                    if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
-                    const int maxload = (strips + 3) / 4;
-                    const double rowEff = (gT * nb / 8.0) / (4.0 * maxload);
-                    int ksc = 0, nst = 0;
-                    if (!choose_pipeline(strips, NT, ksteps, ksc, nst)) continue;
-                    const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
-                    const double fill = ntiles >= 148 ? 1.0 : ntiles / 148.0;
-                    const double lds = 1.0 - 0.03 * (double)(MT + NT) / (MT * NT);
-                    const double score = rowEff * colEff * wf[wi] * lds * (0.5 + 0.5 * fill);
-                    if (score > best + 1e-12) {
-                        best = score;
-                        c.MT = MT; c.NT = NT; c.WM = WM; c.gT = gT; c.wT = wT; c.strips = strips;
-                        c.ksc = ksc; c.nstages = nst;
-                    }
+        for (int MT = 1; MT <= 4; ++MT) {
+            if (MT * NT > kMaxAcc) continue;
+            for (int gT = 1; gT <= n_gamma; ++gT) {
+                const int strips = (gT * nb + 7) / 8;
+                if (strips > MT * WM) break;
+                if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
+                const int maxload = (strips + 3) / 4;
+                const double rowEff = (gT * nb / 8.0) / (4.0 * maxload);
+                int ksc = 0, nst = 0;
+                if (!choose_pipeline(strips, NT, ksteps, ksc, nst)) continue;
+                const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
+                const double fill = ntiles >= 148 ? 1.0 : ntiles / 148.0;
+                const double lds = 1.0 - 0.03 * (double)(MT + NT) / (MT * NT);
+                const double score = rowEff * colEff * lds * (0.5 + 0.5 * fill);
+                if (score > best + 1e-12) {
+                    best = score;
+                    c.MT = MT; c.NT = NT; c.WM = WM; c.gT = gT; c.wT = wT; c.strips = strips;
+                    c.ksc = ksc; c.nstages = nst;
                 }
             }
         }
@@ -662,6 +660,11 @@ int afqmc_get_info(const afqmc_ctx *ctx, afqmc_info *info) {
 }
 
 int afqmc_plan(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, afqmc_info *info) {
+    return afqmc_plan_trial(N, n_alpha, n_beta, n_gamma, max_walkers, 0, 0, info);
+}
+
+int afqmc_plan_trial(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, int complex_alpha, int complex_beta,
+                     afqmc_info *info) {
     if (!info) return fail(nullptr, AFQMC_ERR_ARG, "afqmc_plan: null pointer argument");
     if (N < 1 || n_gamma < 1 || max_walkers < 1 || n_alpha < 0 || n_beta < 0 || n_alpha > N || n_beta > N ||
         n_alpha + n_beta < 1)
@@ -670,8 +673,9 @@ int afqmc_plan(int N, int n_alpha, int n_beta, int n_gamma, int max_walkers, afq
         return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_plan: n_sigma > %d is not supported yet", AFQMC_MAX_NOCC);
     SpinCfg sp[2];
     const int ns[2] = {n_alpha, n_beta};
+    const bool cx[2] = {complex_alpha != 0, complex_beta != 0};
     for (int s = 0; s < 2; ++s)
-        if (!choose_cfg(ns[s], false, N, n_gamma, max_walkers, sp[s]))
+        if (!choose_cfg(ns[s], cx[s], N, n_gamma, max_walkers, sp[s]))
             return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_plan: no K2 tile shape fits n_sigma=%d", ns[s]);
     fill_info(info, N, n_gamma, max_walkers, sp);
     return AFQMC_OK;

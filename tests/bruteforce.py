@@ -162,3 +162,76 @@ def brute_force_greens_function(psi_a, psi_b, phi_a, phi_b, spin):
             if len(b2):
                 G[p, q] = np.sum(np.conj(c_psi[lookup[b2]]) * a2) / ovlp
     return G
+
+
+# ---- dense many-body matrices in the (n_alpha, n_beta) determinant space (tiny systems only) -----------------------
+def determinant_basis(N, na, nb):
+    """Bitstrings of the basis determinants, in the order _minor_expansion produces them."""
+    bits = []
+    for Ia in combinations(range(N), na):
+        ba = sum(1 << p for p in Ia)
+        for Ib in combinations(range(N), nb):
+            bits.append(ba | sum(1 << (N + p) for p in Ib))
+    return np.array(bits, dtype=np.int64)
+
+
+def determinant_vector(phi_a, phi_b, N):
+    """Coefficients of |phi> = prod_j phi+_aj prod_k phi+_bk |0> in determinant_basis order (minors)."""
+    return _minor_expansion(phi_a, phi_b, N)[1]
+
+
+def _operator_matrix(apply, N, na, nb):
+    basis = determinant_basis(N, na, nb)
+    lookup = np.full(1 << (2 * N), -1, dtype=np.int64)
+    lookup[basis] = np.arange(len(basis))
+    M = np.zeros((len(basis), len(basis)), dtype=np.complex128)
+    for col, b in enumerate(basis):
+        for bits, amp in apply(np.array([b], dtype=np.int64), np.array([1.0 + 0j])):
+            if len(bits):
+                np.add.at(M[:, col], lookup[bits], amp)
+    return M
+
+
+def one_body_operator_matrix(A, N, na, nb):
+    """Matrix of sum_{pq,spin} A_pq a+_{p,spin} a_{q,spin} (the same A for both spins) by operator application."""
+    A = np.asarray(A)
+
+    def apply(bits, amp):
+        for so in (0, N):
+            for q in range(N):
+                b1, a1 = _annihilate(bits, amp, so + q)
+                for p in range(N):
+                    if A[p, q] != 0:
+                        b2, a2 = _create(b1, a1, so + p)
+                        yield b2, A[p, q] * a2
+    return _operator_matrix(apply, N, na, nb)
+
+
+def hamiltonian_matrix(h1e, chol, N, na, nb):
+    """Matrix of H of PAPER.md:68 (Eq. 2) with (pr|qs) of Eq. 3, term by term, exactly as brute_force_local_energy
+    applies it (normal-ordered two-body operator a+_p a+_q a_s a_r, no one-body shift)."""
+    V = np.einsum("gpr,gqs->prqs", chol, chol)
+
+    def apply(bits, amp):
+        for so in (0, N):
+            for q in range(N):
+                b1, a1 = _annihilate(bits, amp, so + q)
+                for p in range(N):
+                    b2, a2 = _create(b1, a1, so + p)
+                    yield b2, h1e[p, q] * a2
+        for s1 in (0, N):
+            for r in range(N):
+                b1, a1 = _annihilate(bits, amp, s1 + r)
+                for s2 in (0, N):
+                    for s in range(N):
+                        b2, a2 = _annihilate(b1, a1, s2 + s)
+                        if len(b2) == 0:
+                            continue
+                        for q in range(N):
+                            b3, a3 = _create(b2, a2, s2 + q)
+                            if len(b3) == 0:
+                                continue
+                            for p in range(N):
+                                b4, a4 = _create(b3, a3, s1 + p)
+                                yield b4, 0.5 * V[p, r, q, s] * a4
+    return _operator_matrix(apply, N, na, nb)

@@ -18,6 +18,16 @@ RTOL = 1e-10
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_energies.json")
 
 
+_FULL = {}
+
+
+def _full_inputs(name):
+    """Full-size inputs, generated once per session and per config (`large` takes minutes of host time and 6 GB)."""
+    if name not in _FULL:
+        _FULL[name] = make_inputs(name)
+    return _FULL[name]
+
+
 def _le(inp, max_walkers=None):
     from paper_2209_04015_b200 import LocalEnergy
     dev = "cuda"
@@ -66,7 +76,7 @@ def test_parity_full_size_vs_golden(name):
     and one walker is recomputed live with O3."""
     with open(GOLDEN) as f:
         gold = json.load(f)[name]
-    inp = make_inputs(name)
+    inp = _full_inputs(name)
     assert (gold["N"], gold["n_gamma"], gold["n_walkers"]) == (inp.N, inp.n_gamma, inp.n_walkers)
     E, lo = gpu_energy(inp)
     assert np.all(np.isfinite(E.view(np.float64))) and np.all(np.isfinite(lo.view(np.float64)))
@@ -83,12 +93,12 @@ def test_parity_full_size_vs_golden(name):
     assert_parity(E[[w]], lo[[w]], Eo, loo)
 
 
-@pytest.mark.parametrize("name", ["medium", "cu2o2"])
+@pytest.mark.parametrize("name", ["medium", "cu2o2", "large"])
 def test_parity_every_walker_full_size_vs_listing4(name):
     """Every walker of the full-size launch (not only the sampled ones above) against the paper's half-rotated CPU
     algorithm (oracle/listing4_cpu.py), which tests/test_oracle_pins.py pins to the definition oracle."""
     from oracle.listing4_cpu import HalfRotated, local_energy_listing4
-    inp = make_inputs(name)
+    inp = _full_inputs(name)
     E, lo = gpu_energy(inp)
     hr = HalfRotated(inp.h1e, inp.chol, inp.psi_a, inp.psi_b)
     ref = [local_energy_listing4(hr, inp.e0, inp.phi_a[w], inp.phi_b[w]) for w in range(inp.n_walkers)]
@@ -157,6 +167,41 @@ def test_parity_complex_trial(N, na, nb, ng, nw, which):
     ref = orc.force_bias(inp.chol, inp.psi_a, inp.psi_b, inp.phi_a[0], inp.phi_b[0])
     assert np.all(np.abs(fb.cpu().numpy()[0] - ref) <= 1e-10 * np.max(np.abs(ref)))
     le.close()
+
+
+def _k2_witnesses():
+    from tests.k2_instances import WITNESS
+    return [pytest.param(k, v, id=f"MT{k[0]}_NT{k[1]}") for k, v in sorted(WITNESS.items())]
+
+
+@pytest.mark.parametrize("inst,shape", _k2_witnesses())
+def test_every_k2_instantiation_against_the_oracle(inst, shape):
+    """Every compiled k2_exchange<MT, NT> is launched once (tests/k2_instances.py names a shape the planner maps to
+    it) and compared with the oracle on the first, a middle and the last walker."""
+    n, cx, N, ng, nw = shape
+    inp = _custom(7000 + 100 * inst[0] + inst[1], N, n, 0, ng, nw, complex_trial=bool(cx))
+    le = _le(inp)
+    info = le.info()
+    assert (info["mt"][0], info["nt"][0]) == inst
+    E, lo = gpu_energy(inp, le)
+    le.close()
+    idx = sorted({0, nw // 2, nw - 1})
+    Eo, loo = orc.local_energy_batch(inp, rung="O3", walkers=idx)
+    assert np.all(np.isfinite(E.view(np.float64)))
+    assert_parity(E[idx], lo[idx], Eo, loo)
+
+
+@pytest.mark.parametrize("cx", [False, True], ids=["real", "complex"])
+def test_sweep_over_every_occupation_number(cx):
+    """n_sigma = 1 .. 64 (complex trial: .. 52, the documented limit), unequal spins, N just above n, several gamma tiles
+    and a ragged walker tile: every walker against the oracle."""
+    for n in range(1, 53 if cx else 65):
+        nb = (n * 5) // 7
+        N = max(n + 2, 9)
+        inp = _custom(8000 + n, N, n, nb, 11, 3, complex_trial="both" if cx else False)
+        Eo, loo = orc.local_energy_batch(inp, rung="O3")
+        E, lo = gpu_energy(inp)
+        assert_parity(E, lo, Eo, loo)
 
 
 def test_unequal_spins_sharing_one_kernel_instantiation():

@@ -48,3 +48,27 @@ def test_plan_reports_unsupported_occupation():
 def test_plan_handles_any_occupation(n):
     p = plan(max(n, 70), n, max(n - 1, 0), 50, 9)
     assert p["k2_smem_bytes"][0] <= SMEM_MAX and p["tile_rows"][0] >= n
+
+
+def test_every_compiled_k2_instantiation_has_a_witness_shape():
+    """k2_pick (csrc/afqmc.cu) instantiates k2_exchange<MT, NT> for NT = 1..NTmax(MT); tests/k2_instances.py must name,
+    for each of them, a problem the planner maps to it (the GPU suite launches every row against the oracle)."""
+    import os
+    import re
+    from tests.k2_instances import WITNESS
+    src = open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2209_04015_b200", "csrc",
+                            "afqmc.cu")).read()
+    compiled = set()
+    for mt, ntmax in re.findall(r"case (\d): return k2_pick_nt<\d, (\d+)>\(nt\);", src):
+        compiled |= {(int(mt), nt) for nt in range(1, int(ntmax) + 1)}
+    assert len(compiled) == 43 and compiled == set(WITNESS)
+    for (mt, nt), (n, cx, N, ng, nw) in WITNESS.items():
+        p = plan(N, n, 0, ng, nw, complex_alpha=bool(cx))
+        assert (p["mt"][0], p["nt"][0], p["warps_m"][0]) == (mt, nt, 12), ((mt, nt), p)
+
+
+def test_complex_trial_occupation_limit_is_reported():
+    """A complex trial block stacks Re / Im rows (2 n rows per gamma block): it fits a K2 tile up to n = 52."""
+    plan(60, 52, 3, 10, 4, complex_alpha=True)
+    with pytest.raises(AfqmcError, match="no K2 tile shape"):
+        plan(60, 53, 3, 10, 4, complex_alpha=True)
