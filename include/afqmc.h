@@ -144,13 +144,62 @@ int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream);
  * with afqmc_local_energy / afqmc_force_bias_only:
  *     O = exp(log_ovlp_new - log_ovlp_old),   I = O exp(x . xbar - xbar . xbar / 2),   w_new = |I| max(0, cos(arg O)) w
  *   x             device, float64 [n_walkers][n_gamma]      auxiliary fields drawn by the caller (Eq. 4)
- *   xbar          device, complex128 [n_walkers][n_gamma]   force bias (Eq. 9), e.g. from afqmc_force_bias_only
+ *   xbar          device, complex128 [n_walkers][n_gamma]   the shift of Eq. 9, xbar = -sqrt(dt) <v'>.  NOT the output
+ *                 of afqmc_force_bias[_only], which is Eq. 19's sum_pq G_pq L^g_pq: with the propagator of
+ *                 afqmc_propagate (v' = i v) the two are related by xbar = -i sqrt(dt) * (Eq. 19)
  *   log_ovlp_old/new  device, complex128 [n_walkers]        (log|ovlp|, arg ovlp) as returned in out_overlaps
  *   weights_in/out    device, float64 [n_walkers]           may alias
  * No handle: the call keeps no state.  Enqueued on `stream`.
  */
 int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const void *xbar, const void *log_ovlp_old,
                             const void *log_ovlp_new, const double *weights_in, double *weights_out, void *stream);
+
+/*
+ * afqmc_enable_propagation / afqmc_propagate -- one step of the hybrid phaseless propagation for all walkers
+ * (Eq. 6-13), the other hotspot next to the local energy.
+ *
+ * The paper defines the propagator only through Eq. 4, exp(-dt H) = int dx p(x) B(x) + O(dt^2) with p the normal
+ * distribution.  The reading built here (the oracle pins it with Eq. 4 itself):
+ *     h'       = h - 1/2 sum_g L^g L^g          Eq. 2 is normal ordered: H = sum h'_pq a+_p a_q + 1/2 sum_g v_g^2,
+ *                                               v_g = sum_pr L^g_pr a+_p a_r  (Eq. 2, 3)
+ *     B(dt, y) = exp(-dt h'/2) exp(i sqrt(dt) sum_g y_g L^g) exp(-dt h'/2)     acting on both spin blocks (Eq. 4)
+ *     xbar_g   = -i sqrt(dt) sum_pq G_pq L^g_pq                                Eq. 9 with v' = i v; the sum is Eq. 19
+ *     phi'     = B(dt, x - xbar) phi                                           Eq. 13
+ *     O        = <psi_T|phi'> / <psi_T|phi>                                    Eq. 8
+ *     w'       = |O exp(x.xbar - xbar.xbar/2)| max(0, cos(arg O)) w            Eq. 7, 10-12
+ * No mean-field shift, no population control, no re-orthonormalisation (the paper does not describe them).
+ *
+ * afqmc_enable_propagation(ctx, h1e, chol, dt, stream): one-time setup for time step dt > 0 (fixed per handle).
+ *   h1e, chol   device, the arrays given to afqmc_create (not retained).
+ *   Builds h', exp(-dt h'/2) (scaling and squaring, on the GPU), a third packing of the Cholesky vectors
+ *   (n_gamma * N^2 doubles) as the operand of the field GEMM, the force-bias operand (afqmc_enable_force_bias) and
+ *   work buffers (2 * max_walkers * N^2 doubles for the per-walker matrices sum_g y_g L^g, among others).
+ *   Synchronises `stream`.  A second call on the same handle returns AFQMC_ERR_ARG.
+ *
+ * afqmc_propagate(ctx, walkers, n_walkers, x, weights_in, weights_out, log_ovlp_out, taylor_order, stream):
+ *   walkers       device, complex128, layout of afqmc_local_energy; READ AND OVERWRITTEN with phi' (Eq. 13).
+ *   x             device, float64 [n_walkers][n_gamma]: the auxiliary fields, drawn by the caller from the standard
+ *                 normal distribution (Eq. 4).  The library draws no random numbers.
+ *   weights_in / weights_out   device, float64 [n_walkers]; may alias.
+ *   log_ovlp_out  device, complex128 [n_walkers] or NULL: (log|<psi_T|phi'>|, arg) of the propagated walkers.
+ *   taylor_order  0 .. 64: exp(A) phi is evaluated as sum_{k <= order} A^k phi / k!  (A = i sqrt(dt) sum y_g L^g).  The
+ *                 truncation error, about ||A||^(order+1) / (order+1)!, is the caller's to bound; the paper does not
+ *                 state an order (6 is customary for dt ~ 0.005 and molecular Hamiltonians).
+ *   Kernels, all on `stream`, no host synchronisation: K1 (theta, overlap of phi), force-bias GEMM, field GEMM
+ *   [2 n_walkers x n_gamma].[n_gamma x N^2] on the FP64 tensor cores, order + 2 batched [N x N].[N x 2(n_alpha+n_beta)]
+ *   products, K1 again (overlap of phi'), weight update.  A walker orthogonal to the trial before or after the step gets
+ *   weight NaN (its log-overlap is -inf).  Afterwards the handle's theta belongs to phi' (afqmc_spin_squared,
+ *   afqmc_greens_function refer to the propagated walkers; afqmc_force_bias has nothing to return).
+ *
+ * afqmc_propagation_xbar: copies out the xbar (Eq. 9) of the last afqmc_propagate call, complex128 [n_walkers][n_gamma].
+ * afqmc_propagate_phase_ms: with afqmc_set_profiling(ctx, 1), device times of the last afqmc_propagate call:
+ *   ms[0] K1 + overlap, [1] force-bias GEMM, [2] fields + field GEMM, [3] one-body and Taylor products, [4] K1 + weights.
+ */
+int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *chol, double dt, void *stream);
+int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *x, const double *weights_in,
+                    double *weights_out, void *log_ovlp_out, int taylor_order, void *stream);
+int afqmc_propagation_xbar(afqmc_ctx *ctx, void *out, void *stream);
+int afqmc_propagate_phase_ms(afqmc_ctx *ctx, float ms[5]);
 
 /* Frees the handle and every internal buffer.  NULL is allowed. */
 void afqmc_destroy(afqmc_ctx *ctx);

@@ -16,7 +16,8 @@ _LIB = None
 EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afqmc_force_bias",
            "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_phaseless_weights", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
-           "afqmc_fp64_peak", "afqmc_plan", "afqmc_plan_trial"]
+           "afqmc_fp64_peak", "afqmc_plan", "afqmc_plan_trial", "afqmc_enable_propagation", "afqmc_propagate",
+           "afqmc_propagation_xbar", "afqmc_propagate_phase_ms"]
 
 
 class AfqmcError(RuntimeError):
@@ -82,6 +83,14 @@ def load_library():
     lib.afqmc_plan.restype = ip
     lib.afqmc_plan_trial.argtypes = [ip, ip, ip, ip, ip, ip, ip, C.POINTER(AfqmcInfo)]
     lib.afqmc_plan_trial.restype = ip
+    lib.afqmc_enable_propagation.argtypes = [vp, vp, vp, dp, vp]
+    lib.afqmc_enable_propagation.restype = ip
+    lib.afqmc_propagate.argtypes = [vp, vp, ip, vp, vp, vp, vp, ip, vp]
+    lib.afqmc_propagate.restype = ip
+    lib.afqmc_propagation_xbar.argtypes = [vp, vp, vp]
+    lib.afqmc_propagation_xbar.restype = ip
+    lib.afqmc_propagate_phase_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.afqmc_propagate_phase_ms.restype = ip
     _LIB = lib
     return lib
 
@@ -253,6 +262,51 @@ class LocalEnergy:
                                                     _stream_ptr(stream)), "afqmc_force_bias_only")
         self._last_nw = n_walkers
         return out
+
+    def enable_propagation(self, h1e, chol, dt, stream=None):
+        """afqmc_enable_propagation: one-time setup of the hybrid propagation for time step ``dt`` (CUDA float64 h1e,
+        chol as given at creation)."""
+        for t, cnt in ((h1e, self.N * self.N), (chol, self.n_gamma * self.N * self.N)):
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float64) or t.numel() != cnt:
+                raise AfqmcError("h1e / chol must be the contiguous CUDA float64 tensors given at creation")
+        self._check(self._lib.afqmc_enable_propagation(self._h, h1e.data_ptr(), chol.data_ptr(), float(dt),
+                                                       _stream_ptr(stream)), "afqmc_enable_propagation")
+
+    def propagate(self, walkers, n_walkers, x, weights, taylor_order=6, weights_out=None, log_ovlp_out=None, stream=None):
+        """afqmc_propagate: one hybrid phaseless step (Eq. 6-13).  ``walkers`` (CUDA complex128, ABI layout) is
+        overwritten with the propagated determinants; x float64 [n_walkers, n_gamma]; weights float64 [n_walkers].
+        Returns (weights_out, log_ovlp_out)."""
+        if not (walkers.is_cuda and walkers.is_contiguous() and walkers.dtype == torch.complex128):
+            raise AfqmcError("walkers must be a contiguous CUDA complex128 tensor")
+        if walkers.numel() != n_walkers * self.N * (self.n_alpha + self.n_beta):
+            raise AfqmcError("walkers has the wrong number of elements")
+        for t, cnt in ((x, n_walkers * self.n_gamma), (weights, n_walkers)):
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float64) or t.numel() != cnt:
+                raise AfqmcError("x / weights must be contiguous CUDA float64 tensors of [n_walkers, n_gamma] / [n_walkers]")
+        if weights_out is None:
+            weights_out = torch.empty(n_walkers, dtype=torch.float64, device=walkers.device)
+        if log_ovlp_out is None:
+            log_ovlp_out = torch.empty(n_walkers, dtype=torch.complex128, device=walkers.device)
+        for t, dt_ in ((weights_out, torch.float64), (log_ovlp_out, torch.complex128)):
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == dt_) or t.numel() != n_walkers:
+                raise AfqmcError("weights_out / log_ovlp_out must be contiguous CUDA tensors of n_walkers elements")
+        rc = self._lib.afqmc_propagate(self._h, walkers.data_ptr(), n_walkers, x.data_ptr(), weights.data_ptr(),
+                                       weights_out.data_ptr(), log_ovlp_out.data_ptr(), int(taylor_order),
+                                       _stream_ptr(stream))
+        self._check(rc, "afqmc_propagate")
+        self._last_nw, self._last_energy_nw = n_walkers, 0
+        return weights_out, log_ovlp_out
+
+    def propagation_xbar(self, out=None, stream=None):
+        """afqmc_propagation_xbar: the shift xbar (Eq. 9) of the last propagate call, complex128 [n_walkers, n_gamma]."""
+        out = self._out_for_last_call("propagation_xbar", None, self._last_nw, (self.n_gamma,), out)
+        self._check(self._lib.afqmc_propagation_xbar(self._h, out.data_ptr(), _stream_ptr(stream)), "afqmc_propagation_xbar")
+        return out
+
+    def propagate_phase_ms(self):
+        ms = (C.c_float * 5)()
+        self._check(self._lib.afqmc_propagate_phase_ms(self._h, ms), "afqmc_propagate_phase_ms")
+        return [float(v) for v in ms]
 
     def spin_squared(self, n_walkers=None, out=None, stream=None):
         """afqmc_spin_squared: [n_walkers] complex128 <S^2> mixed estimator for the walkers of the last energy /

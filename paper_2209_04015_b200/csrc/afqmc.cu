@@ -22,6 +22,7 @@
 #include "k5_spin_squared.cuh"
 #include "k6_greens.cuh"
 #include "k7_phaseless.cuh"
+#include "k8_propagate.cuh"
 
 using namespace afqmc;
 
@@ -74,6 +75,19 @@ struct afqmc_ctx {
     int last_nw = 0;                   // walkers whose theta the handle holds (last energy or force-bias-only call)
     int last_energy_nw = 0;            // walkers whose Coulomb traces the handle holds (last energy call)
     bool fb_enabled = false;
+    // propagation (afqmc_enable_propagation): one-body factor, field-GEMM operands, work buffers
+    bool prop_enabled = false;
+    double dt = 0.0;
+    int ldE = 0, ldt = 0, p_rt_strips = 0, p_row_tiles = 0;      // pitches of E / of the working walker layout; K9 row tiling
+    double *hp = nullptr, *Emat = nullptr, *Etmp[2] = {nullptr, nullptr};
+    int v_strips = 0, v_n_ct = 0, v_kps = 0, v_ksc = 0, v_nchunks = 0, v_nstages = 0;
+    size_t v_smem = 0;
+    long long ldv = 0;
+    OperandLayout v_layA{}, v_layB{};
+    double *v_A = nullptr, *v_B = nullptr, *V = nullptr, *fbuf = nullptr, *xbar = nullptr, *Tb[3] = {nullptr, nullptr, nullptr};
+    double *lo_old = nullptr, *lo_new = nullptr;
+    cudaEvent_t pev[8] = {};           // per-phase events of the last profiled afqmc_propagate
+    bool pev_valid = false;
     long long launches = 0;
     bool profiling = false;
     std::vector<cudaEvent_t> ev;       // kProfSets x 4 events, created by the first afqmc_set_profiling(1)
@@ -234,6 +248,10 @@ void free_ctx(afqmc_ctx *c) {
         cudaFree(c->sp[s].tbuf); cudaFree(c->sp[s].xpart);
     }
     cudaFree(c->e1); cudaFree(c->logdet); cudaFree(c->h_walkers); cudaFree(c->h_outE); cudaFree(c->h_outO);
+    cudaFree(c->hp); cudaFree(c->Emat); cudaFree(c->Etmp[0]); cudaFree(c->Etmp[1]); cudaFree(c->v_A); cudaFree(c->v_B);
+    cudaFree(c->V); cudaFree(c->fbuf); cudaFree(c->xbar); cudaFree(c->Tb[0]); cudaFree(c->Tb[1]); cudaFree(c->Tb[2]);
+    cudaFree(c->lo_old); cudaFree(c->lo_new);
+    for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     for (auto &e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
 }
@@ -278,6 +296,53 @@ int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, 
     size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
     if (with_fb) k1_overlap_inverse_theta<true><<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
     else k1_overlap_inverse_theta<false><<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+// The force-bias GEMM (one launch per spin) and the combine kernel, on the theta K1<with_fb> has just written.
+int launch_force_bias_gemm(afqmc_ctx *ctx, int n_walkers, double *out, cudaStream_t stream) {
+    K4Params p4{};
+    p4.n_walkers = n_walkers; p4.n_gamma = ctx->n_gamma; p4.out = out;
+    for (int s = 0; s < 2; ++s) {
+        const SpinCfg &sc = ctx->sp[s];
+        p4.n[s] = sc.n;
+        if (sc.n == 0) continue;
+        const int nbf = sc.cplx ? 2 : 1;
+        K2FbParams p2{};
+        p2.A = sc.f_A; p2.B = sc.f_B;
+        p2.itemA_doubles = sc.f_layA.tile_doubles / sc.f_ksplit;   // parts of a tile are contiguous
+        p2.tileB_doubles = sc.f_layB.tile_doubles;
+        p2.partB_doubles = (long long)sc.f_kps * sc.f_NT * 32;
+        p2.rows_per_tile = sc.f_gT * nbf; p2.rows_total = ctx->n_gamma * nbf;
+        p2.strips = sc.f_strips; p2.WM = K2_MAX_WM;
+        p2.kps = sc.f_kps; p2.ksc = sc.f_ksc; p2.nchunks = sc.f_nchunks; p2.nstages = sc.f_nstages;
+        p2.n_items_r = sc.f_n_rt * sc.f_ksplit; p2.ksplit = sc.f_ksplit; p2.n_ct = (n_walkers + sc.f_wT - 1) / sc.f_wT;
+        p2.craw = sc.f_craw;
+        const long long ntiles = (long long)p2.n_items_r * p2.n_ct;
+        const int grid = (int)std::min<long long>(ntiles, ctx->num_sms);
+        K2FbFn fn = k2_pick_fb(sc.f_NT);
+        fn<<<grid, 32 * K2_MAX_WM, sc.f_smem, stream>>>(p2);
+        CU_TRY(ctx, cudaGetLastError());
+        ctx->launches += 1;
+        p4.nb[s] = nbf; p4.wT[s] = sc.f_wT; p4.n_ct[s] = p2.n_ct; p4.ldc[s] = sc.f_NT * 8; p4.craw[s] = sc.f_craw; p4.ksplit[s] = sc.f_ksplit;
+    }
+    const long long total = (long long)n_walkers * ctx->n_gamma;
+    k4_force_bias_combine<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(p4);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+// One K9 launch: Out_b = alpha M_b In_b (+ Sum_b), b = 0 .. batch-1.
+int launch_k9(afqmc_ctx *ctx, const double *Mre, const double *Mim, long long m_stride, int ldm, const double *In, double *Out,
+              double *Sum, long long io_stride, int ld, int C, int batch, double alpha, cudaStream_t stream) {
+    K9Params p{};
+    p.Mre = Mre; p.Mim = Mim; p.m_batch_stride = m_stride; p.ldm = ldm; p.In = In; p.Out = Out; p.Sum = Sum;
+    p.io_batch_stride = io_stride; p.ld = ld; p.N = ctx->N; p.C = C; p.rt_strips = ctx->p_rt_strips; p.alpha = alpha;
+    const dim3 grid(ctx->p_row_tiles, (C + K9_NT * 8 - 1) / (K9_NT * 8), batch);
+    k9_apply<<<grid, K9_THREADS, K9_SMEM, stream>>>(p);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;
@@ -551,35 +616,7 @@ int afqmc_force_bias_only(afqmc_ctx *ctx, const void *walkers, int n_walkers, vo
         return fail(ctx, AFQMC_ERR_ARG, "afqmc_force_bias_only: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
     cudaStream_t stream = (cudaStream_t)stream_;
     if (int rc = launch_k1(ctx, walkers, n_walkers, true, stream)) return rc;
-    K4Params p4{};
-    p4.n_walkers = n_walkers; p4.n_gamma = ctx->n_gamma; p4.out = reinterpret_cast<double *>(out);
-    for (int s = 0; s < 2; ++s) {
-        const SpinCfg &sc = ctx->sp[s];
-        p4.n[s] = sc.n;
-        if (sc.n == 0) continue;
-        const int nbf = sc.cplx ? 2 : 1;
-        K2FbParams p2{};
-        p2.A = sc.f_A; p2.B = sc.f_B;
-        p2.itemA_doubles = sc.f_layA.tile_doubles / sc.f_ksplit;   // parts of a tile are contiguous
-        p2.tileB_doubles = sc.f_layB.tile_doubles;
-        p2.partB_doubles = (long long)sc.f_kps * sc.f_NT * 32;
-        p2.rows_per_tile = sc.f_gT * nbf; p2.rows_total = ctx->n_gamma * nbf;
-        p2.strips = sc.f_strips; p2.WM = K2_MAX_WM;
-        p2.kps = sc.f_kps; p2.ksc = sc.f_ksc; p2.nchunks = sc.f_nchunks; p2.nstages = sc.f_nstages;
-        p2.n_items_r = sc.f_n_rt * sc.f_ksplit; p2.ksplit = sc.f_ksplit; p2.n_ct = (n_walkers + sc.f_wT - 1) / sc.f_wT;
-        p2.craw = sc.f_craw;
-        const long long ntiles = (long long)p2.n_items_r * p2.n_ct;
-        const int grid = (int)std::min<long long>(ntiles, ctx->num_sms);
-        K2FbFn fn = k2_pick_fb(sc.f_NT);
-        fn<<<grid, 32 * K2_MAX_WM, sc.f_smem, stream>>>(p2);
-        CU_TRY(ctx, cudaGetLastError());
-        ctx->launches += 1;
-        p4.nb[s] = nbf; p4.wT[s] = sc.f_wT; p4.n_ct[s] = p2.n_ct; p4.ldc[s] = sc.f_NT * 8; p4.craw[s] = sc.f_craw; p4.ksplit[s] = sc.f_ksplit;
-    }
-    const long long total = (long long)n_walkers * ctx->n_gamma;
-    k4_force_bias_combine<<<(unsigned)((total + 255) / 256), 256, 0, stream>>>(p4);
-    CU_TRY(ctx, cudaGetLastError());
-    ctx->launches += 1;
+    if (int rc = launch_force_bias_gemm(ctx, n_walkers, reinterpret_cast<double *>(out), stream)) return rc;
     ctx->last_nw = n_walkers;
     return AFQMC_OK;
 }
@@ -631,6 +668,189 @@ int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const v
         n_gamma, x, reinterpret_cast<const double *>(xbar), reinterpret_cast<const double *>(log_ovlp_old),
         reinterpret_cast<const double *>(log_ovlp_new), weights_in, weights_out);
     CU_TRY(nullptr, cudaGetLastError());
+    return AFQMC_OK;
+}
+
+int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *chol, double dt, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!h1e || !chol) return fail(ctx, AFQMC_ERR_ARG, "afqmc_enable_propagation: null pointer argument");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(ctx, AFQMC_ERR_ARG, "afqmc_enable_propagation: dt must be positive and finite");
+    if (ctx->prop_enabled) return fail(ctx, AFQMC_ERR_ARG, "afqmc_enable_propagation: already enabled on this handle (dt = %g)", ctx->dt);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (int rc = afqmc_enable_force_bias(ctx, chol, stream_)) return rc;
+    const int N = ctx->N, n_gamma = ctx->n_gamma, maxw = ctx->maxw;
+    const int C = 2 * (ctx->sp[0].n + ctx->sp[1].n);
+    ctx->dt = dt;
+    ctx->ldE = (N + 1) & ~1; ctx->ldt = C;                        // even pitches: K9 stores (re, im) pairs as double2
+    const int S = (N + 7) / 8;
+    ctx->p_row_tiles = (S + 2 * K9_WARPS - 1) / (2 * K9_WARPS);
+    ctx->p_rt_strips = (S + ctx->p_row_tiles - 1) / ctx->p_row_tiles;
+    CU_TRY(ctx, allow_max_smem(k9_apply));
+    CU_TRY(ctx, allow_max_smem(k2_force_bias<16>));
+
+    // ---- h' = h - 1/2 sum_g (L^g)^2 and E = exp(-dt h'/2) by scaling and squaring (all products in K9) -------------
+    const size_t ebytes = (size_t)N * ctx->ldE * 8;
+    CU_TRY(ctx, cudaMalloc(&ctx->hp, (size_t)N * N * 8));
+    CU_TRY(ctx, cudaMalloc(&ctx->Emat, ebytes));
+    CU_TRY(ctx, cudaMalloc(&ctx->Etmp[0], ebytes));
+    CU_TRY(ctx, cudaMalloc(&ctx->Etmp[1], ebytes));
+    k8_one_body_shift<<<dim3((N + 15) / 16, (N + 15) / 16), 256, 0, stream>>>(h1e, chol, N, n_gamma, ctx->hp);
+    CU_TRY(ctx, cudaGetLastError());
+    std::vector<double> hp_h((size_t)N * N);
+    CU_TRY(ctx, cudaMemcpyAsync(hp_h.data(), ctx->hp, hp_h.size() * 8, cudaMemcpyDeviceToHost, stream));
+    CU_TRY(ctx, cudaStreamSynchronize(stream));
+    double norm1 = 0.0;                                           // picks the number of squarings only
+    for (int q = 0; q < N; ++q) {
+        double c = 0.0;
+        for (int p = 0; p < N; ++p) c += std::fabs(hp_h[(size_t)p * N + q]);
+        norm1 = std::max(norm1, c);
+    }
+    if (!std::isfinite(norm1)) return fail(ctx, AFQMC_ERR_ARG, "afqmc_enable_propagation: h1e / chol have non-finite entries");
+    int nsq = 0;
+    while (0.5 * dt * norm1 / std::ldexp(1.0, nsq) > 0.5 && nsq < 60) ++nsq;
+    double *term = ctx->Etmp[0], *next = ctx->Etmp[1], *sum = ctx->Emat;
+    CU_TRY(ctx, cudaMemsetAsync(term, 0, ebytes, stream));
+    CU_TRY(ctx, cudaMemsetAsync(next, 0, ebytes, stream));
+    CU_TRY(ctx, cudaMemsetAsync(sum, 0, ebytes, stream));
+    k8_set_diagonal<<<(N + 255) / 256, 256, 0, stream>>>(term, N, ctx->ldE, 1.0);
+    k8_set_diagonal<<<(N + 255) / 256, 256, 0, stream>>>(sum, N, ctx->ldE, 1.0);
+    CU_TRY(ctx, cudaGetLastError());
+    for (int k = 1; k <= 18; ++k) {                               // ||X|| <= 1/2: the 18th term is below 1e-21
+        const double alpha = -0.5 * dt / std::ldexp(1.0, nsq) / k;
+        if (int rc = launch_k9(ctx, ctx->hp, nullptr, 0, N, term, next, sum, 0, ctx->ldE, N, 1, alpha, stream)) return rc;
+        std::swap(term, next);
+    }
+    double *cur = sum, *other = term;                             // `term` and `next` are free now
+    for (int k = 0; k < nsq; ++k) {
+        if (int rc = launch_k9(ctx, cur, nullptr, 0, ctx->ldE, cur, other, nullptr, 0, ctx->ldE, N, 1, 1.0, stream)) return rc;
+        std::swap(cur, other);
+    }
+    if (cur != ctx->Emat) CU_TRY(ctx, cudaMemcpyAsync(ctx->Emat, cur, ebytes, cudaMemcpyDeviceToDevice, stream));
+
+    // ---- operands of the field GEMM  A(y)_w[pq] = sum_g c_wg L^g[pq] ------------------------------------------------
+    const int ksteps = (n_gamma + 3) / 4;
+    ctx->v_ksc = std::min(12, ksteps);
+    ctx->v_kps = (ksteps + ctx->v_ksc - 1) / ctx->v_ksc * ctx->v_ksc;
+    ctx->v_nchunks = ctx->v_kps / ctx->v_ksc;
+    ctx->v_nstages = 2;
+    const int rstrips = (2 * maxw + 7) / 8, rtiles = (rstrips + K2_MAX_WM - 1) / K2_MAX_WM;
+    ctx->v_strips = (rstrips + rtiles - 1) / rtiles;
+    const long long npq = (long long)N * N;
+    ctx->v_n_ct = (int)((npq + 127) / 128);
+    ctx->ldv = (long long)ctx->v_n_ct * 128;
+    ctx->v_smem = (size_t)ctx->v_nstages * ctx->v_ksc * (ctx->v_strips + 16) * 256 + (size_t)2 * ctx->v_nstages * 8 + 16;
+    ctx->v_layA = OperandLayout{1, ctx->v_strips, ctx->v_kps, ctx->v_strips * 8, (long long)ctx->v_strips * ctx->v_kps * 32};
+    ctx->v_layB = OperandLayout{1, 16, ctx->v_kps, 128, (long long)16 * ctx->v_kps * 32};
+    const size_t a_bytes = (size_t)rtiles * ctx->v_layA.tile_doubles * 8, b_bytes = (size_t)ctx->v_n_ct * ctx->v_layB.tile_doubles * 8;
+    CU_TRY(ctx, cudaMalloc(&ctx->v_A, a_bytes));
+    CU_TRY(ctx, cudaMalloc(&ctx->v_B, b_bytes));
+    CU_TRY(ctx, cudaMemsetAsync(ctx->v_A, 0, a_bytes, stream));
+    CU_TRY(ctx, cudaMemsetAsync(ctx->v_B, 0, b_bytes, stream));
+    k8_pack_chol_vhs<<<dim3((unsigned)((npq + 255) / 256), ksteps), 256, 0, stream>>>(chol, npq, n_gamma, ctx->v_layB, ctx->v_B);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 4 + 18 + nsq;
+
+    // ---- work buffers ------------------------------------------------------------------------------------------------
+    CU_TRY(ctx, cudaMalloc(&ctx->V, (size_t)2 * maxw * ctx->ldv * 8));
+    CU_TRY(ctx, cudaMalloc(&ctx->fbuf, (size_t)maxw * n_gamma * 16));
+    CU_TRY(ctx, cudaMalloc(&ctx->xbar, (size_t)maxw * n_gamma * 16));
+    for (int k = 0; k < 3; ++k) CU_TRY(ctx, cudaMalloc(&ctx->Tb[k], (size_t)maxw * N * ctx->ldt * 8));
+    CU_TRY(ctx, cudaMalloc(&ctx->lo_old, (size_t)maxw * 16));
+    CU_TRY(ctx, cudaMalloc(&ctx->lo_new, (size_t)maxw * 16));
+    for (auto &e : ctx->pev) CU_TRY(ctx, cudaEventCreate(&e));
+    CU_TRY(ctx, cudaStreamSynchronize(stream));
+    ctx->prop_enabled = true;
+    return AFQMC_OK;
+}
+
+int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *x, const double *weights_in,
+                    double *weights_out, void *log_ovlp_out, int taylor_order, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!walkers || !x || !weights_in || !weights_out) return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagate: null pointer argument");
+    if (!ctx->prop_enabled) return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagate: call afqmc_enable_propagation first");
+    if (n_walkers < 1 || n_walkers > ctx->maxw)
+        return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagate: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
+    if (taylor_order < 0 || taylor_order > 64) return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagate: taylor_order=%d outside 0..64", taylor_order);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int N = ctx->N, n_gamma = ctx->n_gamma, na = ctx->sp[0].n, nb = ctx->sp[1].n, C = 2 * (na + nb), ld = ctx->ldt;
+    const long long tstride = (long long)N * ld;
+    cudaEvent_t *ev = ctx->profiling ? ctx->pev : nullptr;
+    int evi = 0;
+    auto mark = [&]() -> cudaError_t { return ev ? cudaEventRecord(ev[evi++], stream) : cudaSuccess; };
+    CU_TRY(ctx, mark());
+
+    // (1) theta, log-overlap of phi (Eq. 16, 23) and the force bias sum_pq G_pq L^g_pq (Eq. 19 / 24)
+    if (int rc = launch_k1(ctx, walkers, n_walkers, true, stream)) return rc;
+    k8_log_overlap<<<(n_walkers + 127) / 128, 128, 0, stream>>>(n_walkers, ctx->maxw, na, nb, ctx->logdet, ctx->lo_old);
+    CU_TRY(ctx, cudaGetLastError());
+    CU_TRY(ctx, mark());
+    if (int rc = launch_force_bias_gemm(ctx, n_walkers, ctx->fbuf, stream)) return rc;
+    CU_TRY(ctx, mark());
+
+    // (2) xbar (Eq. 9) and the coefficients of A(x - xbar); A(y)_w = sum_g c_wg L^g on the FP64 tensor cores
+    const long long nf = (long long)n_walkers * ((n_gamma + 3) / 4);
+    k8_fields<<<(unsigned)((nf + 255) / 256), 256, 0, stream>>>(n_walkers, n_gamma, ctx->dt, ctx->fbuf, x, ctx->xbar, ctx->v_layA, ctx->v_A);
+    CU_TRY(ctx, cudaGetLastError());
+    {
+        K2FbParams p2{};
+        p2.A = ctx->v_A; p2.B = ctx->v_B;
+        p2.itemA_doubles = ctx->v_layA.tile_doubles; p2.tileB_doubles = ctx->v_layB.tile_doubles; p2.partB_doubles = 0;
+        p2.rows_per_tile = ctx->v_strips * 8; p2.rows_total = 2 * n_walkers;
+        p2.strips = ctx->v_strips; p2.WM = K2_MAX_WM;
+        p2.kps = ctx->v_kps; p2.ksc = ctx->v_ksc; p2.nchunks = ctx->v_nchunks; p2.nstages = ctx->v_nstages;
+        p2.n_items_r = (2 * n_walkers + p2.rows_per_tile - 1) / p2.rows_per_tile; p2.ksplit = 1; p2.n_ct = ctx->v_n_ct;
+        p2.craw = ctx->V;
+        const long long ntiles = (long long)p2.n_items_r * p2.n_ct;
+        k2_force_bias<16><<<(int)std::min<long long>(ntiles, ctx->num_sms), 32 * K2_MAX_WM, ctx->v_smem, stream>>>(p2);
+        CU_TRY(ctx, cudaGetLastError());
+    }
+    CU_TRY(ctx, mark());
+
+    // (3) phi' = E exp(A) E phi (Eq. 13): T0 = E phi, S = sum_k A^k T0 / k!, phi' = E S
+    double *X0 = ctx->Tb[0], *X1 = ctx->Tb[1], *X2 = ctx->Tb[2];
+    const long long np = (long long)n_walkers * N * ld;
+    k8_pack_walkers<<<(unsigned)((np + 255) / 256), 256, 0, stream>>>(reinterpret_cast<const double *>(walkers), n_walkers, N, na, nb, ld, X0);
+    CU_TRY(ctx, cudaGetLastError());
+    if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, X0, X1, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;
+    CU_TRY(ctx, cudaMemcpyAsync(X0, X1, (size_t)np * 8, cudaMemcpyDeviceToDevice, stream));          // running sum S = T0
+    double *cur = X1, *nxt = X2;
+    for (int k = 1; k <= taylor_order; ++k) {
+        if (int rc = launch_k9(ctx, ctx->V, ctx->V + ctx->ldv, 2 * ctx->ldv, N, cur, nxt, X0, tstride, ld, C, n_walkers, 1.0 / k, stream)) return rc;
+        std::swap(cur, nxt);
+    }
+    if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, X0, cur, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;
+    const long long nu = (long long)n_walkers * N * C;
+    k8_unpack_walkers<<<(unsigned)((nu + 255) / 256), 256, 0, stream>>>(cur, n_walkers, N, na, nb, ld, reinterpret_cast<double *>(walkers));
+    CU_TRY(ctx, cudaGetLastError());
+    CU_TRY(ctx, mark());
+
+    // (4) overlap of phi' (Eq. 8) and the phaseless weights (Eq. 7, 10-12)
+    if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream)) return rc;
+    k8_log_overlap<<<(n_walkers + 127) / 128, 128, 0, stream>>>(n_walkers, ctx->maxw, na, nb, ctx->logdet, ctx->lo_new);
+    CU_TRY(ctx, cudaGetLastError());
+    k7_phaseless_update<<<n_walkers, K7_THREADS, 0, stream>>>(n_gamma, x, ctx->xbar, ctx->lo_old, ctx->lo_new, weights_in, weights_out);
+    CU_TRY(ctx, cudaGetLastError());
+    if (log_ovlp_out) CU_TRY(ctx, cudaMemcpyAsync(log_ovlp_out, ctx->lo_new, (size_t)n_walkers * 16, cudaMemcpyDeviceToDevice, stream));
+    CU_TRY(ctx, mark());
+    ctx->pev_valid = ev != nullptr;
+    ctx->launches += 9 + taylor_order;
+    ctx->last_nw = n_walkers;
+    ctx->last_energy_nw = 0;            // the Coulomb traces in the handle belong to other walkers now
+    return AFQMC_OK;
+}
+
+int afqmc_propagate_phase_ms(afqmc_ctx *ctx, float ms[5]) {
+    if (!ctx || !ms) return AFQMC_ERR_ARG;
+    if (!ctx->pev_valid) return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagate_phase_ms: no profiled afqmc_propagate call recorded");
+    for (int k = 0; k < 5; ++k) CU_TRY(ctx, cudaEventElapsedTime(&ms[k], ctx->pev[k], ctx->pev[k + 1]));
+    return AFQMC_OK;
+}
+
+int afqmc_propagation_xbar(afqmc_ctx *ctx, void *out, void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!out) return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagation_xbar: null pointer argument");
+    if (!ctx->prop_enabled || ctx->last_nw < 1) return fail(ctx, AFQMC_ERR_ARG, "afqmc_propagation_xbar: no afqmc_propagate call has been made");
+    CU_TRY(ctx, cudaMemcpyAsync(out, ctx->xbar, (size_t)ctx->last_nw * ctx->n_gamma * 16, cudaMemcpyDeviceToDevice, (cudaStream_t)stream_));
     return AFQMC_OK;
 }
 

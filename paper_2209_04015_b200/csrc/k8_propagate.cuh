@@ -1,0 +1,293 @@
+// K8 / K9 -- one step of the hybrid phaseless propagation (Eq. 4, Eq. 6-13).
+//
+// The paper gives the propagator only through Eq. 4.  The reading built here (rows 17-19):
+//     H = sum h'_pq a+_p a_q + 1/2 sum_g v_g^2 ,   v_g = sum_pr L^g_pr a+_p a_r ,   h' = h - 1/2 sum_g (L^g)^2      (Eq. 2, 3)
+//     B(dt, y) = exp(-dt h'/2) exp(A(y)) exp(-dt h'/2) ,   A(y) = i sqrt(dt) sum_g y_g L^g                          (Eq. 4)
+//     xbar_g   = -i sqrt(dt) sum_pq G_pq L^g_pq   (Eq. 9 with v' = i v; the sum is Eq. 19 / 24's force bias)
+//     phi'     = B(dt, x - xbar) phi  (Eq. 13),   exp(A) phi by its Taylor series truncated at a caller-chosen order.
+//
+// Kernels (all FP64; the two GEMM-shaped steps run on DMMA.8x8x4):
+//   k8_one_body_shift      h' = h - 1/2 sum_g L^g L^g                                  once per handle
+//   k8_pack_chol_vhs       chol [g][pq] -> B operand of the field GEMM (fragment order) once per handle
+//   k8_fields              xbar, and the coefficients c_g = i sqrt(dt) (x_g - xbar_g) of A(y) as the GEMM's A operand
+//   (k2_force_bias<16>)    A(y)_w[pq] = sum_g c_wg L^g[pq]  -- a real GEMM [2 Nw x Ngamma].[Ngamma x N^2] over the
+//                          same TMA-fed operand ring as the force-bias GEMM (k2_exchange.cuh)
+//   k9_apply               Out_w = alpha M_w In_w (+ running sum), M complex (planes) or real and shared: the Taylor terms
+//                          A T_k / (k+1), the one-body factors exp(-dt h'/2) T, and the squarings that build exp(-dt h'/2)
+//   k8_pack_walkers / k8_unpack_walkers   ABI walker layout <-> [w][p][(spin, j, re/im)] working layout
+//   k8_log_overlap         sum over spins of K1's log-determinants, arg wrapped to (-pi, pi]
+#pragma once
+#include <math_constants.h>
+#include "common.cuh"
+
+namespace afqmc {
+
+// ------------------------------------------------------------------------------------------------------------------
+// h' = h - 1/2 sum_g L^g L^g.  grid (ceil(N/16), ceil(N/16)), block 16 x 16; gamma looped inside.  One-time.
+__global__ void __launch_bounds__(256) k8_one_body_shift(const double *__restrict__ h1e, const double *__restrict__ chol, int N,
+                                                         int n_gamma, double *__restrict__ hp) {
+    __shared__ double a[16][17], b[16][17];
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    const int p = blockIdx.y * 16 + ty, q = blockIdx.x * 16 + tx;
+    double acc = 0.0;
+    for (int g = 0; g < n_gamma; ++g) {
+        const double *L = chol + (size_t)g * N * N;
+        for (int r0 = 0; r0 < N; r0 += 16) {
+            a[ty][tx] = (p < N && r0 + tx < N) ? L[(size_t)p * N + r0 + tx] : 0.0;
+            b[ty][tx] = (r0 + ty < N && q < N) ? L[(size_t)(r0 + ty) * N + q] : 0.0;
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 16; ++r) acc = fma(a[ty][r], b[r][tx], acc);
+            __syncthreads();
+        }
+    }
+    if (p < N && q < N) hp[(size_t)p * N + q] = h1e[(size_t)p * N + q] - 0.5 * acc;
+}
+
+// chol [g][pq] -> packed B operand: tile = pq / (8 strips), strip, lane = (pq % 8) * 4 + g % 4, k-step = g / 4.
+// One thread per (group of 4 gamma, pq): reads are coalesced along pq, each thread writes one 32-byte run.
+__global__ void k8_pack_chol_vhs(const double *__restrict__ chol, long long npq, int n_gamma, OperandLayout lay,
+                                 double *__restrict__ packed) {
+    const long long pq = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int g0 = blockIdx.y * 4;
+    if (pq >= npq) return;
+    const int cols_per_tile = lay.strips * 8;
+    const int tile = (int)(pq / cols_per_tile), c = (int)(pq - (long long)tile * cols_per_tile);
+    double v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = (g0 + k < n_gamma) ? chol[(size_t)(g0 + k) * npq + pq] : 0.0;
+    double *dst = packed + packed_offset(lay, tile, c, g0);
+    *reinterpret_cast<double2 *>(dst) = make_double2(v[0], v[1]);
+    *reinterpret_cast<double2 *>(dst + 2) = make_double2(v[2], v[3]);
+}
+
+// xbar_wg = -i sqrt(dt) fb_wg (Eq. 9);  c_wg = i sqrt(dt) (x_wg - xbar_wg) = -dt fb_wg + i sqrt(dt) x_wg.
+// Writes xbar [Nw][Ngamma] complex and the GEMM's A operand: row 2w = Re c_w, row 2w + 1 = Im c_w, k = gamma.
+__global__ void k8_fields(int n_walkers, int n_gamma, double dt, const double *__restrict__ fb /* [Nw][Ng][2] */,
+                          const double *__restrict__ x /* [Nw][Ng] */, double *__restrict__ xbar, OperandLayout lay,
+                          double *__restrict__ packedA) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int g4 = (n_gamma + 3) / 4;
+    if (idx >= (long long)n_walkers * g4) return;
+    const int w = (int)(idx / g4), g0 = (int)(idx - (long long)w * g4) * 4;
+    const double sdt = sqrt(dt);
+    double cr[4], ci[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int g = g0 + k;
+        cr[k] = 0.0; ci[k] = 0.0;
+        if (g < n_gamma) {
+            const double fr = fb[((long long)w * n_gamma + g) * 2], fi = fb[((long long)w * n_gamma + g) * 2 + 1];
+            const double xv = x[(long long)w * n_gamma + g];
+            xbar[((long long)w * n_gamma + g) * 2] = sdt * fi;          // -i sqrt(dt) (fr + i fi) = sqrt(dt) fi - i sqrt(dt) fr
+            xbar[((long long)w * n_gamma + g) * 2 + 1] = -sdt * fr;
+            cr[k] = -dt * fr;
+            ci[k] = sdt * xv - dt * fi;
+        }
+    }
+    const int rows_per_tile = lay.strips * 8;
+#pragma unroll
+    for (int plane = 0; plane < 2; ++plane) {
+        const int row = 2 * w + plane;
+        const int tile = row / rows_per_tile;
+        double *dst = packedA + packed_offset(lay, tile, row - tile * rows_per_tile, g0);
+        const double *v = plane ? ci : cr;
+        *reinterpret_cast<double2 *>(dst) = make_double2(v[0], v[1]);
+        *reinterpret_cast<double2 *>(dst + 2) = make_double2(v[2], v[3]);
+    }
+}
+
+// ABI walkers (alpha block [Nw][N][na] then beta block [Nw][N][nb], complex) <-> working layout T[w][p][ld]:
+// real column 2 j + c for alpha orbital j, 2 na + 2 j + c for beta orbital j (c = 0 re, 1 im); columns >= C are zero.
+__global__ void k8_pack_walkers(const double *__restrict__ walkers, int n_walkers, int N, int na, int nb, int ld,
+                                double *__restrict__ T) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)n_walkers * N * ld) return;
+    const int col = (int)(idx % ld);
+    const long long wp = idx / ld;
+    const int p = (int)(wp % N), w = (int)(wp / N);
+    double v = 0.0;
+    if (col < 2 * na) v = walkers[(((long long)w * N + p) * na) * 2 + col];
+    else if (col < 2 * (na + nb)) v = walkers[(long long)n_walkers * N * na * 2 + (((long long)w * N + p) * nb) * 2 + (col - 2 * na)];
+    T[idx] = v;
+}
+
+__global__ void k8_unpack_walkers(const double *__restrict__ T, int n_walkers, int N, int na, int nb, int ld,
+                                  double *__restrict__ walkers) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int C = 2 * (na + nb);
+    if (idx >= (long long)n_walkers * N * C) return;
+    const int col = (int)(idx % C);
+    const long long wp = idx / C;
+    const int p = (int)(wp % N), w = (int)(wp / N);
+    const double v = T[wp * ld + col];
+    if (col < 2 * na) walkers[(((long long)w * N + p) * na) * 2 + col] = v;
+    else walkers[(long long)n_walkers * N * na * 2 + (((long long)w * N + p) * nb) * 2 + (col - 2 * na)] = v;
+}
+
+// log-overlap of a walker = sum over spins of K1's (log|det S|, arg det S), arg wrapped to (-pi, pi]   (Eq. 16)
+__global__ void k8_log_overlap(int n_walkers, int maxw, int na, int nb, const double *__restrict__ logdet /* [2][maxw][2] */,
+                               double *__restrict__ out /* [Nw][2] */) {
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_walkers) return;
+    double la = 0.0, ar = 0.0;
+    if (na > 0) { la += logdet[(long long)w * 2]; ar += logdet[(long long)w * 2 + 1]; }
+    if (nb > 0) { la += logdet[((long long)maxw + w) * 2]; ar += logdet[((long long)maxw + w) * 2 + 1]; }
+    if (ar > CUDART_PI) ar -= 2.0 * CUDART_PI;
+    else if (ar <= -CUDART_PI) ar += 2.0 * CUDART_PI;
+    out[2 * w] = la; out[2 * w + 1] = ar;
+}
+
+// identity * s into an [N][ld] matrix that has been zeroed
+__global__ void k8_set_diagonal(double *M, int N, int ld, double s) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < N) M[(size_t)p * ld + p] = s;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// K9: Out_b = alpha * M_b * In_b  (and Sum_b += Out_b),  b = batch (walker).
+//   M_b: N x N, complex given as two planes (Mre, Mim, row pitch ldm) or real (Mim == nullptr); m_batch_stride = 0
+//        shares one M between all batches (the one-body factor exp(-dt h'/2)).
+//   In_b / Out_b / Sum_b: N x ld real, columns are (re, im)-interleaved complex columns when M is complex:
+//        (Mre + i Mim) T = Mre T + Mim (i T),   (i T)[q][2m] = -T[q][2m+1],  (i T)[q][2m+1] = T[q][2m],
+//        so one accumulator set takes both products; the C fragment of DMMA.8x8x4 holds (re, im) of one complex entry.
+// Tiling: grid (row tiles, column groups of <= 104 columns, batch), 12 warps, warp w owns strips w and w + 12 of the row
+// tile (rt_strips <= 24) and all <= 13 column blocks (K2's register shape: 2 x 13 accumulator tiles per warp); the q range is staged through shared memory in chunks of 16 by
+// 8-byte cp.async, double buffered.  Pitches 20 / 116 doubles (= 4 mod 16) make the fragment loads conflict free.
+constexpr int K9_THREADS = 384;
+constexpr int K9_WARPS = K9_THREADS / 32;
+constexpr int K9_KC = 16;             // q per chunk = 4 DMMA k-steps
+constexpr int K9_MAXROWS = 192;       // 24 strips
+constexpr int K9_NT = 13;             // column blocks per group
+constexpr int K9_APITCH = 20, K9_BPITCH = 116;
+constexpr int K9_SMEM = 2 * (2 * K9_MAXROWS * K9_APITCH + K9_KC * K9_BPITCH) * 8;
+
+struct K9Params {
+    const double *Mre, *Mim;
+    long long m_batch_stride;
+    int ldm;
+    const double *In;
+    double *Out, *Sum;               // Sum may be nullptr
+    long long io_batch_stride;
+    int ld;                          // even
+    int N, C;                        // M is N x N; In has C real columns in use
+    int rt_strips;                   // strips per row tile (<= 24)
+    double alpha;
+};
+
+__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src, bool valid) {
+    const int sz = valid ? 8 : 0;    // src-size 0: the 8 destination bytes are zero-filled
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_u32(dst_smem)), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_) : "memory"); }
+
+__global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads x 168 registers = the register file
+    extern __shared__ __align__(16) unsigned char k9_smem[];
+    double *sA = reinterpret_cast<double *>(k9_smem);                          // [2 stages][2 planes][192][20]
+    double *sB = sA + 2 * 2 * K9_MAXROWS * K9_APITCH;                          // [2 stages][16][116]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int N = P.N, b = blockIdx.z;
+    const int row0 = blockIdx.x * P.rt_strips * 8;
+    const int rows = min(P.rt_strips * 8, N - row0);                           // valid rows of this tile
+    const int col0 = blockIdx.y * (K9_NT * 8);
+    const int ncols = min(K9_NT * 8, P.C - col0);
+    const int nt = (ncols + 7) >> 3;
+    const bool cplx = P.Mim != nullptr;
+    const double *Mre = P.Mre + (long long)b * P.m_batch_stride;
+    const double *Mim = cplx ? P.Mim + (long long)b * P.m_batch_stride : nullptr;
+    const double *In = P.In + (long long)b * P.io_batch_stride;
+    const int nplanes = cplx ? 2 : 1;
+    const int my_mt = (warp + K9_WARPS < P.rt_strips) ? 2 : (warp < P.rt_strips ? 1 : 0);
+
+    auto load_chunk = [&](int stage, int q0) {
+        double *a = sA + stage * (2 * K9_MAXROWS * K9_APITCH);
+        double *bb = sB + stage * (K9_KC * K9_BPITCH);
+        const int arows = P.rt_strips * 8;
+        for (int e = tid; e < nplanes * arows * K9_KC; e += K9_THREADS) {
+            const int k = e & (K9_KC - 1), r = (e / K9_KC) % arows, pl = e / (K9_KC * arows);
+            const bool ok = (r < rows) && (q0 + k < N);
+            const double *src = (pl ? Mim : Mre) + (ok ? (long long)(row0 + r) * P.ldm + q0 + k : 0);
+            cp_async8(a + (pl * K9_MAXROWS + r) * K9_APITCH + k, src, ok);
+        }
+        const int bcols = nt * 8;
+        for (int e = tid; e < K9_KC * bcols; e += K9_THREADS) {
+            const int c = e % bcols, k = e / bcols;
+            const bool ok = (q0 + k < N) && (c < ncols);
+            const double *src = In + (ok ? (long long)(q0 + k) * P.ld + col0 + c : 0);
+            cp_async8(bb + k * K9_BPITCH + c, src, ok);
+        }
+        cp_async_commit();
+    };
+
+    double acc[2][K9_NT][2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m)
+#pragma unroll
+        for (int q = 0; q < K9_NT; ++q) { acc[m][q][0] = 0.0; acc[m][q][1] = 0.0; }
+
+    const int nchunks = (N + K9_KC - 1) / K9_KC;
+    load_chunk(0, 0);
+    const int fr = lane >> 2, fk = lane & 3;
+    const double sgn = (fr & 1) ? 1.0 : -1.0;                                  // (i T)[q][c] = sgn * T[q][c ^ 1]
+    for (int ch = 0; ch < nchunks; ++ch) {
+        if (ch + 1 < nchunks) { load_chunk((ch + 1) & 1, (ch + 1) * K9_KC); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncthreads();
+        const double *a = sA + (ch & 1) * (2 * K9_MAXROWS * K9_APITCH);
+        const double *bb = sB + (ch & 1) * (K9_KC * K9_BPITCH);
+        if (my_mt > 0) {
+#pragma unroll
+            for (int ks = 0; ks < K9_KC / 4; ++ks) {
+                double are[2], aim[2];
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                    const int r = (warp + K9_WARPS * m) * 8 + fr;
+                    are[m] = (m < my_mt) ? a[r * K9_APITCH + ks * 4 + fk] : 0.0;
+                    aim[m] = (cplx && m < my_mt) ? a[(K9_MAXROWS + r) * K9_APITCH + ks * 4 + fk] : 0.0;
+                }
+#pragma unroll
+                for (int q = 0; q < K9_NT; ++q) {
+                    if (q < nt) {
+                        const double *bp = bb + (ks * 4 + fk) * K9_BPITCH + q * 8;
+                        const double b0 = bp[fr];
+                        dmma_m8n8k4(acc[0][q][0], acc[0][q][1], are[0], b0);
+                        if (my_mt > 1) dmma_m8n8k4(acc[1][q][0], acc[1][q][1], are[1], b0);
+                        if (cplx) {
+                            const double b1 = sgn * bp[fr ^ 1];
+                            dmma_m8n8k4(acc[0][q][0], acc[0][q][1], aim[0], b1);
+                            if (my_mt > 1) dmma_m8n8k4(acc[1][q][0], acc[1][q][1], aim[1], b1);
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    double *Out = P.Out + (long long)b * P.io_batch_stride;
+    double *Sum = P.Sum ? P.Sum + (long long)b * P.io_batch_stride : nullptr;
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+        if (m >= my_mt) continue;
+        const int r = (warp + K9_WARPS * m) * 8 + fr;
+        if (r >= rows) continue;
+#pragma unroll
+        for (int q = 0; q < K9_NT; ++q) {
+            const int c = q * 8 + 2 * fk;
+            if (q < nt && c < ncols) {                                          // ld is even and C is even or padded: (c, c+1) stay inside the row
+                const long long off = (long long)(row0 + r) * P.ld + col0 + c;
+                const double2 v = make_double2(P.alpha * acc[m][q][0], P.alpha * acc[m][q][1]);
+                *reinterpret_cast<double2 *>(Out + off) = v;
+                if (Sum) {
+                    double2 s = *reinterpret_cast<double2 *>(Sum + off);
+                    s.x += v.x; s.y += v.y;
+                    *reinterpret_cast<double2 *>(Sum + off) = s;
+                }
+            }
+        }
+    }
+}
+
+}  // namespace afqmc
