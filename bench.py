@@ -150,6 +150,7 @@ def main():
     ap.add_argument("--config", default="cu2o2", choices=["tiny", "small", "medium", "cu2o2", "large"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-propagation", action="store_true", help="skip the propagation-step leg (SURVEY 8f-4)")
     ap.add_argument("--all-configs", action="store_true",
                     help="also time the other four configs (device-resident, fewer steps) and add them as "
                          "'other_configs' to the JSON line; generating 'large' takes a few minutes of host time")
@@ -196,6 +197,10 @@ def main():
     trial = torch.from_numpy(inp.trial_packed()).to(dev)
     le = LocalEnergy(h1e, chol, trial, inp.N, inp.n_alpha, inp.n_beta, inp.n_gamma, inp.e0, nw)
     le.enable_force_bias(chol)          # operand of the dedicated force-bias GEMM (reported under "force_bias")
+    PROP_DT, PROP_ORDER = 0.0001, 6     # customary Taylor order; 1/50 of the paper's Cu2O2 time step
+    # because the synthetic Cholesky vectors are ~100x a molecule's: at 0.005 the overlap ratio overflows exp()
+    if not args.no_propagation:
+        le.enable_propagation(h1e, chol, PROP_DT)
     del chol
     torch.cuda.empty_cache()
     walkers_host = torch.from_numpy(inp.walkers_packed()).pin_memory()
@@ -260,6 +265,43 @@ def main():
     ms_fb = max_over_ranks(e0.elapsed_time(e1)) / args.steps
     flops_fb = 4.0 * inp.N * inp.n_gamma * nw * (inp.n_alpha + inp.n_beta)
 
+    # ---- one hybrid propagation step: K1, force bias, field GEMM, Taylor, K1, weights --
+    prop = None
+    if not args.no_propagation:
+        gen = torch.Generator(device=dev)
+        gen.manual_seed(1234 + rank)
+        xf = torch.randn((nw, inp.n_gamma), dtype=torch.float64, device=dev, generator=gen)
+        wts = torch.ones(nw, dtype=torch.float64, device=dev)
+        wts_out, lo_out = torch.empty_like(wts), torch.empty(nw, dtype=torch.complex128, device=dev)
+        wk = walkers.clone()
+        le.set_profiling(True)
+        for _ in range(3):
+            wk.copy_(walkers)
+            le.propagate(wk, nw, xf, wts, PROP_ORDER, wts_out, lo_out)
+        barrier()
+        phase = np.zeros(5)
+        e0.record(stream)
+        for _ in range(args.steps):
+            wk.copy_(walkers)               # every step starts from the same determinants (62 MB device copy, timed)
+            le.propagate(wk, nw, xf, wts, PROP_ORDER, wts_out, lo_out)
+        e1.record(stream)
+        barrier()
+        phase = np.array(le.propagate_phase_ms())          # phases of the last step
+        le.set_profiling(False)
+        ms_prop = max_over_ranks(e0.elapsed_time(e1)) / args.steps
+        ne = inp.n_alpha + inp.n_beta
+        flops_field = 4.0 * nw * inp.n_gamma * inp.N * (inp.N + 1) / 2         # [2Nw x Ng].[Ng x N(N+1)/2] real GEMM (L symmetric)
+        flops_taylor = (PROP_ORDER * 8.0 + 2 * 4.0) * inp.N ** 2 * ne * nw      # complex A T_k terms + two real E T products
+        prop = {"value": world * nw / (ms_prop * 1e-3), "unit": UNIT, "ms_per_step": ms_prop, "dt": PROP_DT,
+                "taylor_order": PROP_ORDER,
+                "what": "afqmc_propagate: K1 + force-bias GEMM + field GEMM [2Nw x Ng].[Ng x N(N+1)/2] + (order + 2) batched "
+                        "[N x N].[N x 2(na+nb)] products + K1 + phaseless weights; device-resident, x drawn beforehand",
+                "phase_ms": {"k1_overlap": phase[0], "force_bias_gemm": phase[1], "fields_and_field_gemm": phase[2],
+                             "one_body_and_taylor": phase[3], "k1_and_weights": phase[4]},
+                "field_gemm": {"algorithmic_flops": flops_field, "tflops": flops_field / (phase[2] * 1e-3) * 1e-12},
+                "taylor": {"algorithmic_flops": flops_taylor, "tflops": flops_taylor / (phase[3] * 1e-3) * 1e-12},
+                "finite": bool(torch.isfinite(wts_out).all().item())}
+
     # ---- roofline of K2 -------------------------------------------------------------------------------------
     nspin_launches = int(inp.n_alpha > 0) + int(inp.n_beta > 0)
     flops_k2 = 4.0 * inp.N * inp.n_gamma * nw * (inp.n_alpha ** 2 + inp.n_beta ** 2)        # per step, both spins
@@ -267,6 +309,9 @@ def main():
     k2_launch_ms = kms[1] / nspin_launches
     achieved = flops_per_launch / (k2_launch_ms * 1e-3) * 1e-12
     peak = max(peak_dmma, peak_dfma)
+    if prop is not None:
+        prop["field_gemm"]["frac_of_fp64_peak"] = prop["field_gemm"]["tflops"] / peak
+        prop["taylor"]["frac_of_fp64_peak"] = prop["taylor"]["tflops"] / peak
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "k2_dram_traffic.json")
     if os.path.exists(tpath):
@@ -395,6 +440,7 @@ def main():
                                "algorithmic_flops_per_step": flops_fb,
                                "tflops_incl_k1": flops_fb / (ms_fb * 1e-3) * 1e-12,
                                "speedup_vs_energy_step": (ms_total / args.steps) / ms_fb},
+                "propagation": prop,
                 "roofline": roofline,
                 "cpu_baseline": cpu,
                 "cpu_baseline_listing4": cpu_b}

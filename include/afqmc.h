@@ -172,8 +172,8 @@ int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const v
  * afqmc_enable_propagation(ctx, h1e, chol, dt, stream): one-time setup for time step dt > 0 (fixed per handle).
  *   h1e, chol   device, the arrays given to afqmc_create (not retained).
  *   Builds h', exp(-dt h'/2) (scaling and squaring, on the GPU), a third packing of the Cholesky vectors
- *   (n_gamma * N^2 doubles) as the operand of the field GEMM, the force-bias operand (afqmc_enable_force_bias) and
- *   work buffers (2 * max_walkers * N^2 doubles for the per-walker matrices sum_g y_g L^g, among others).
+ *   (upper triangles only, n_gamma * N (N + 1) / 2 doubles: every L^g is symmetric) as the operand of the field GEMM, the force-bias operand (afqmc_enable_force_bias) and
+ *   work buffers (3 * max_walkers * N^2 doubles for the per-walker matrices sum_g y_g L^g, among others).
  *   Synchronises `stream`.  A second call on the same handle returns AFQMC_ERR_ARG.
  *
  * afqmc_propagate(ctx, walkers, n_walkers, x, weights_in, weights_out, log_ovlp_out, taylor_order, stream):
@@ -186,7 +186,7 @@ int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const v
  *                 truncation error, about ||A||^(order+1) / (order+1)!, is the caller's to bound; the paper does not
  *                 state an order (6 is customary for dt ~ 0.005 and molecular Hamiltonians).
  *   Kernels, all on `stream`, no host synchronisation: K1 (theta, overlap of phi), force-bias GEMM, field GEMM
- *   [2 n_walkers x n_gamma].[n_gamma x N^2] on the FP64 tensor cores, order + 2 batched [N x N].[N x 2(n_alpha+n_beta)]
+ *   [2 n_walkers x n_gamma].[n_gamma x N(N+1)/2] on the FP64 tensor cores, order + 2 batched [N x N].[N x 2(n_alpha+n_beta)]
  *   products, K1 again (overlap of phi'), weight update.  A walker orthogonal to the trial before or after the step gets
  *   weight NaN (its log-overlap is -inf).  Afterwards the handle's theta belongs to phi' (afqmc_spin_squared,
  *   afqmc_greens_function refer to the propagated walkers; afqmc_force_bias has nothing to return).

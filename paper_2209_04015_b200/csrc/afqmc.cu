@@ -84,7 +84,7 @@ struct afqmc_ctx {
     size_t v_smem = 0;
     long long ldv = 0;
     OperandLayout v_layA{}, v_layB{};
-    double *v_A = nullptr, *v_B = nullptr, *V = nullptr, *fbuf = nullptr, *xbar = nullptr, *Tb[3] = {nullptr, nullptr, nullptr};
+    double *v_A = nullptr, *v_B = nullptr, *V = nullptr, *Vtri = nullptr, *fbuf = nullptr, *xbar = nullptr, *Tb[3] = {nullptr, nullptr, nullptr};
     double *lo_old = nullptr, *lo_new = nullptr;
     cudaEvent_t pev[8] = {};           // per-phase events of the last profiled afqmc_propagate
     bool pev_valid = false;
@@ -249,7 +249,7 @@ void free_ctx(afqmc_ctx *c) {
     }
     cudaFree(c->e1); cudaFree(c->logdet); cudaFree(c->h_walkers); cudaFree(c->h_outE); cudaFree(c->h_outO);
     cudaFree(c->hp); cudaFree(c->Emat); cudaFree(c->Etmp[0]); cudaFree(c->Etmp[1]); cudaFree(c->v_A); cudaFree(c->v_B);
-    cudaFree(c->V); cudaFree(c->fbuf); cudaFree(c->xbar); cudaFree(c->Tb[0]); cudaFree(c->Tb[1]); cudaFree(c->Tb[2]);
+    cudaFree(c->V); cudaFree(c->Vtri); cudaFree(c->fbuf); cudaFree(c->xbar); cudaFree(c->Tb[0]); cudaFree(c->Tb[1]); cudaFree(c->Tb[2]);
     cudaFree(c->lo_old); cudaFree(c->lo_new);
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     for (auto &e : c->ev) if (e) cudaEventDestroy(e);
@@ -341,7 +341,12 @@ int launch_k9(afqmc_ctx *ctx, const double *Mre, const double *Mim, long long m_
     K9Params p{};
     p.Mre = Mre; p.Mim = Mim; p.m_batch_stride = m_stride; p.ldm = ldm; p.In = In; p.Out = Out; p.Sum = Sum;
     p.io_batch_stride = io_stride; p.ld = ld; p.N = ctx->N; p.C = C; p.rt_strips = ctx->p_rt_strips; p.alpha = alpha;
-    const dim3 grid(ctx->p_row_tiles, (C + K9_NT * 8 - 1) / (K9_NT * 8), batch);
+    // column groups: as few as fit the accumulators, of equal width (splitting further to fill the last wave of CTAs was
+    // measured and lost: 5.6 vs 4.7 ms for the Taylor phase at cu2o2, the M tile is then staged twice)
+    const int blocks = (C + 7) / 8;
+    const int groups = (blocks + K9_NT - 1) / K9_NT;
+    p.cg_blocks = (blocks + groups - 1) / groups;
+    const dim3 grid(ctx->p_row_tiles, (blocks + p.cg_blocks - 1) / p.cg_blocks, batch);
     k9_apply<<<grid, K9_THREADS, K9_SMEM, stream>>>(p);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
@@ -735,7 +740,7 @@ int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *ch
     ctx->v_nstages = 2;
     const int rstrips = (2 * maxw + 7) / 8, rtiles = (rstrips + K2_MAX_WM - 1) / K2_MAX_WM;
     ctx->v_strips = (rstrips + rtiles - 1) / rtiles;
-    const long long npq = (long long)N * N;
+    const long long npq = (long long)N * (N + 1) / 2;             // upper triangle: L^g and A(y) are symmetric
     ctx->v_n_ct = (int)((npq + 127) / 128);
     ctx->ldv = (long long)ctx->v_n_ct * 128;
     ctx->v_smem = (size_t)ctx->v_nstages * ctx->v_ksc * (ctx->v_strips + 16) * 256 + (size_t)2 * ctx->v_nstages * 8 + 16;
@@ -746,12 +751,14 @@ int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *ch
     CU_TRY(ctx, cudaMalloc(&ctx->v_B, b_bytes));
     CU_TRY(ctx, cudaMemsetAsync(ctx->v_A, 0, a_bytes, stream));
     CU_TRY(ctx, cudaMemsetAsync(ctx->v_B, 0, b_bytes, stream));
-    k8_pack_chol_vhs<<<dim3((unsigned)((npq + 255) / 256), ksteps), 256, 0, stream>>>(chol, npq, n_gamma, ctx->v_layB, ctx->v_B);
+    if (ksteps > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_enable_propagation: n_gamma > 262140 is not supported");
+    k8_pack_chol_vhs<<<dim3((N + 127) / 128, N, ksteps), 128, 0, stream>>>(chol, N, n_gamma, ctx->v_layB, ctx->v_B);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 4 + 18 + nsq;
 
     // ---- work buffers ------------------------------------------------------------------------------------------------
-    CU_TRY(ctx, cudaMalloc(&ctx->V, (size_t)2 * maxw * ctx->ldv * 8));
+    CU_TRY(ctx, cudaMalloc(&ctx->Vtri, (size_t)2 * maxw * ctx->ldv * 8));
+    CU_TRY(ctx, cudaMalloc(&ctx->V, (size_t)2 * maxw * N * N * 8));
     CU_TRY(ctx, cudaMalloc(&ctx->fbuf, (size_t)maxw * n_gamma * 16));
     CU_TRY(ctx, cudaMalloc(&ctx->xbar, (size_t)maxw * n_gamma * 16));
     for (int k = 0; k < 3; ++k) CU_TRY(ctx, cudaMalloc(&ctx->Tb[k], (size_t)maxw * N * ctx->ldt * 8));
@@ -799,9 +806,12 @@ int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *
         p2.strips = ctx->v_strips; p2.WM = K2_MAX_WM;
         p2.kps = ctx->v_kps; p2.ksc = ctx->v_ksc; p2.nchunks = ctx->v_nchunks; p2.nstages = ctx->v_nstages;
         p2.n_items_r = (2 * n_walkers + p2.rows_per_tile - 1) / p2.rows_per_tile; p2.ksplit = 1; p2.n_ct = ctx->v_n_ct;
-        p2.craw = ctx->V;
+        p2.craw = ctx->Vtri;
         const long long ntiles = (long long)p2.n_items_r * p2.n_ct;
         k2_force_bias<16><<<(int)std::min<long long>(ntiles, ctx->num_sms), 32 * K2_MAX_WM, ctx->v_smem, stream>>>(p2);
+        CU_TRY(ctx, cudaGetLastError());
+        if (2 * n_walkers > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_propagate: more than 32767 walkers per call");
+        k8_expand_symmetric<<<dim3((N + 127) / 128, N, 2 * n_walkers), 128, 0, stream>>>(ctx->Vtri, ctx->ldv, N, ctx->V);
         CU_TRY(ctx, cudaGetLastError());
     }
     CU_TRY(ctx, mark());
@@ -815,7 +825,7 @@ int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *
     CU_TRY(ctx, cudaMemcpyAsync(X0, X1, (size_t)np * 8, cudaMemcpyDeviceToDevice, stream));          // running sum S = T0
     double *cur = X1, *nxt = X2;
     for (int k = 1; k <= taylor_order; ++k) {
-        if (int rc = launch_k9(ctx, ctx->V, ctx->V + ctx->ldv, 2 * ctx->ldv, N, cur, nxt, X0, tstride, ld, C, n_walkers, 1.0 / k, stream)) return rc;
+        if (int rc = launch_k9(ctx, ctx->V, ctx->V + (long long)N * N, 2LL * N * N, N, cur, nxt, X0, tstride, ld, C, n_walkers, 1.0 / k, stream)) return rc;
         std::swap(cur, nxt);
     }
     if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, X0, cur, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;
@@ -833,7 +843,7 @@ int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *
     if (log_ovlp_out) CU_TRY(ctx, cudaMemcpyAsync(log_ovlp_out, ctx->lo_new, (size_t)n_walkers * 16, cudaMemcpyDeviceToDevice, stream));
     CU_TRY(ctx, mark());
     ctx->pev_valid = ev != nullptr;
-    ctx->launches += 9 + taylor_order;
+    ctx->launches += 10 + taylor_order;
     ctx->last_nw = n_walkers;
     ctx->last_energy_nw = 0;            // the Coulomb traces in the handle belong to other walkers now
     return AFQMC_OK;

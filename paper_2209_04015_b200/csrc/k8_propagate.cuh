@@ -8,10 +8,11 @@
 //
 // Kernels (all FP64; the two GEMM-shaped steps run on DMMA.8x8x4):
 //   k8_one_body_shift      h' = h - 1/2 sum_g L^g L^g                                  once per handle
-//   k8_pack_chol_vhs       chol [g][pq] -> B operand of the field GEMM (fragment order) once per handle
+//   k8_pack_chol_vhs       chol [g][p<=q] -> B operand of the field GEMM (fragment order, upper triangle only) once per handle
 //   k8_fields              xbar, and the coefficients c_g = i sqrt(dt) (x_g - xbar_g) of A(y) as the GEMM's A operand
-//   (k2_force_bias<16>)    A(y)_w[pq] = sum_g c_wg L^g[pq]  -- a real GEMM [2 Nw x Ngamma].[Ngamma x N^2] over the
+//   (k2_force_bias<16>)    A(y)_w[p<=q] = sum_g c_wg L^g[pq]  -- a real GEMM [2 Nw x Ngamma].[Ngamma x N(N+1)/2] over the
 //                          same TMA-fed operand ring as the force-bias GEMM (k2_exchange.cuh)
+//   k8_expand_symmetric    upper triangle -> full N x N planes for K9
 //   k9_apply               Out_w = alpha M_w In_w (+ running sum), M complex (planes) or real and shared: the Taylor terms
 //                          A T_k / (k+1), the one-body factors exp(-dt h'/2) T, and the squarings that build exp(-dt h'/2)
 //   k8_pack_walkers / k8_unpack_walkers   ABI walker layout <-> [w][p][(spin, j, re/im)] working layout
@@ -44,21 +45,35 @@ __global__ void __launch_bounds__(256) k8_one_body_shift(const double *__restric
     if (p < N && q < N) hp[(size_t)p * N + q] = h1e[(size_t)p * N + q] - 0.5 * acc;
 }
 
-// chol [g][pq] -> packed B operand: tile = pq / (8 strips), strip, lane = (pq % 8) * 4 + g % 4, k-step = g / 4.
-// One thread per (group of 4 gamma, pq): reads are coalesced along pq, each thread writes one 32-byte run.
-__global__ void k8_pack_chol_vhs(const double *__restrict__ chol, long long npq, int n_gamma, OperandLayout lay,
+// Every L^g is symmetric (Eq. 3; "ipie exploits symmetry in the Cholesky tensor to reduce its memory footprint",
+// PAPER.md:469), so A(y) is too: the field GEMM only produces the upper triangle, t(p, q) = p N - p (p - 1) / 2 + q - p
+// for p <= q, N (N + 1) / 2 columns instead of N^2 -- half the flops and half the third packing of chol.
+__host__ __device__ inline long long tri_index(int p, int q, int N) { return (long long)p * N - (long long)p * (p - 1) / 2 + (q - p); }
+
+// chol [g][p][q], q >= p -> packed B operand: column t(p, q), tile = t / (8 strips), lane = (t % 8) * 4 + g % 4, k-step = g / 4.
+// grid (ceil(N/128), N, ceil(Ngamma/4)): one thread per (p, q, group of 4 gamma); reads coalesced along q, 32-byte writes.
+__global__ void k8_pack_chol_vhs(const double *__restrict__ chol, int N, int n_gamma, OperandLayout lay,
                                  double *__restrict__ packed) {
-    const long long pq = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int g0 = blockIdx.y * 4;
-    if (pq >= npq) return;
+    const int q = blockIdx.x * blockDim.x + threadIdx.x, p = blockIdx.y, g0 = blockIdx.z * 4;
+    if (q >= N || q < p) return;
+    const long long t = tri_index(p, q, N);
     const int cols_per_tile = lay.strips * 8;
-    const int tile = (int)(pq / cols_per_tile), c = (int)(pq - (long long)tile * cols_per_tile);
+    const int tile = (int)(t / cols_per_tile), c = (int)(t - (long long)tile * cols_per_tile);
     double v[4];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = (g0 + k < n_gamma) ? chol[(size_t)(g0 + k) * npq + pq] : 0.0;
+    for (int k = 0; k < 4; ++k) v[k] = (g0 + k < n_gamma) ? chol[((size_t)(g0 + k) * N + p) * N + q] : 0.0;
     double *dst = packed + packed_offset(lay, tile, c, g0);
     *reinterpret_cast<double2 *>(dst) = make_double2(v[0], v[1]);
     *reinterpret_cast<double2 *>(dst + 2) = make_double2(v[2], v[3]);
+}
+
+// Upper triangle [row][ldtri] -> full symmetric matrices [row][N][N]  (row = 2 w + plane).  grid (ceil(N/128), N, rows).
+__global__ void k8_expand_symmetric(const double *__restrict__ tri, long long ldtri, int N, double *__restrict__ full) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x, p = blockIdx.y;
+    if (q >= N) return;
+    const long long row = blockIdx.z;
+    const long long t = p <= q ? tri_index(p, q, N) : tri_index(q, p, N);
+    full[(row * N + p) * N + q] = tri[row * ldtri + t];
 }
 
 // xbar_wg = -i sqrt(dt) fb_wg (Eq. 9);  c_wg = i sqrt(dt) (x_wg - xbar_wg) = -dt fb_wg + i sqrt(dt) x_wg.
@@ -172,12 +187,14 @@ struct K9Params {
     int ld;                          // even
     int N, C;                        // M is N x N; In has C real columns in use
     int rt_strips;                   // strips per row tile (<= 24)
+    int cg_blocks;                   // 8-column blocks per column group (<= K9_NT); grid.y groups cover C
     double alpha;
 };
 
-__device__ __forceinline__ void cp_async8(void *dst_smem, const void *src, bool valid) {
-    const int sz = valid ? 8 : 0;    // src-size 0: the 8 destination bytes are zero-filled
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_u32(dst_smem)), "l"(src), "r"(sz) : "memory");
+// cp.async of BYTES (8 or 16) with `valid` source bytes (0 .. BYTES); the rest of the destination is zero-filled.
+template <int BYTES>
+__device__ __forceinline__ void cp_async_zfill(void *dst_smem, const void *src, int valid) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;\n" ::"r"(smem_u32(dst_smem)), "l"(src), "n"(BYTES), "r"(valid) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N_>
@@ -191,8 +208,8 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
     const int N = P.N, b = blockIdx.z;
     const int row0 = blockIdx.x * P.rt_strips * 8;
     const int rows = min(P.rt_strips * 8, N - row0);                           // valid rows of this tile
-    const int col0 = blockIdx.y * (K9_NT * 8);
-    const int ncols = min(K9_NT * 8, P.C - col0);
+    const int col0 = blockIdx.y * (P.cg_blocks * 8);
+    const int ncols = min(P.cg_blocks * 8, P.C - col0);
     const int nt = (ncols + 7) >> 3;
     const bool cplx = P.Mim != nullptr;
     const double *Mre = P.Mre + (long long)b * P.m_batch_stride;
@@ -201,22 +218,43 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
     const int nplanes = cplx ? 2 : 1;
     const int my_mt = (warp + K9_WARPS < P.rt_strips) ? 2 : (warp < P.rt_strips ? 1 : 0);
 
+    // Per-thread copy duties, fixed over the chunk loop (no index arithmetic per chunk).
+    //   M rows: 16-byte pieces when every row start is 16-byte aligned (ldm even), else 8-byte pieces.
+    //   In rows: always 16-byte pieces (ld and the column offsets are even).
+    const bool avec = ((P.ldm & 1) == 0) && ((reinterpret_cast<uintptr_t>(Mre) & 15) == 0) &&
+                      (!cplx || (reinterpret_cast<uintptr_t>(Mim) & 15) == 0);
+    const int a_piece = avec ? (tid & 7) * 2 : (tid & 15), a_r0 = avec ? (tid >> 3) : (tid >> 4), a_rstep = avec ? 48 : 24;
+    const int bpieces = nt * 4;                                                // 16-byte pieces per q row of In
+    int b_k[3], b_c[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int e = tid + j * K9_THREADS;
+        b_k[j] = e < K9_KC * bpieces ? e / bpieces : -1;
+        b_c[j] = (e - (e / bpieces) * bpieces) * 2;
+    }
+
     auto load_chunk = [&](int stage, int q0) {
         double *a = sA + stage * (2 * K9_MAXROWS * K9_APITCH);
         double *bb = sB + stage * (K9_KC * K9_BPITCH);
-        const int arows = P.rt_strips * 8;
-        for (int e = tid; e < nplanes * arows * K9_KC; e += K9_THREADS) {
-            const int k = e & (K9_KC - 1), r = (e / K9_KC) % arows, pl = e / (K9_KC * arows);
-            const bool ok = (r < rows) && (q0 + k < N);
-            const double *src = (pl ? Mim : Mre) + (ok ? (long long)(row0 + r) * P.ldm + q0 + k : 0);
-            cp_async8(a + (pl * K9_MAXROWS + r) * K9_APITCH + k, src, ok);
+        const int qa = q0 + a_piece;
+        for (int pl = 0; pl < nplanes; ++pl) {
+            const double *M = pl ? Mim : Mre;
+            for (int r = a_r0; r < P.rt_strips * 8; r += a_rstep) {
+                const bool rok = r < rows;
+                double *dst = a + (pl * K9_MAXROWS + r) * K9_APITCH + a_piece;
+                const double *src = M + (rok ? (long long)(row0 + r) * P.ldm + min(qa, N - 1) : 0);
+                if (avec) cp_async_zfill<16>(dst, src, rok ? max(0, min(2, N - qa)) * 8 : 0);
+                else cp_async_zfill<8>(dst, src, (rok && qa < N) ? 8 : 0);
+            }
         }
-        const int bcols = nt * 8;
-        for (int e = tid; e < K9_KC * bcols; e += K9_THREADS) {
-            const int c = e % bcols, k = e / bcols;
-            const bool ok = (q0 + k < N) && (c < ncols);
-            const double *src = In + (ok ? (long long)(q0 + k) * P.ld + col0 + c : 0);
-            cp_async8(bb + k * K9_BPITCH + c, src, ok);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            if (b_k[j] >= 0) {
+                const int q = q0 + b_k[j];
+                const int vb = q < N ? max(0, min(2, ncols - b_c[j])) * 8 : 0;
+                const double *src = In + (vb ? (long long)q * P.ld + col0 + b_c[j] : 0);
+                cp_async_zfill<16>(bb + b_k[j] * K9_BPITCH + b_c[j], src, vb);
+            }
         }
         cp_async_commit();
     };
