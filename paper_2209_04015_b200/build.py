@@ -7,14 +7,32 @@ import subprocess
 PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB = os.path.join(PKG_DIR, "libafqmc.so")
+OZAKI_LIB = os.path.join(PKG_DIR, "libafqmc_ozaki.so")       # the Ozaki-scheme experiment (include/afqmc_ozaki.h)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 
 
 def _sources():
-    out = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh"))]
+    out = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh")) and f != "ozaki_i8.cu"]
     out.append(os.path.join(os.path.dirname(PKG_DIR), "include", "afqmc.h"))
     return out
+
+
+def _nvcc():
+    nvcc = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
+    return nvcc if os.path.exists(nvcc) else "nvcc"
+
+
+def build_ozaki_library(force: bool = False) -> str:
+    """Compile csrc/ozaki_i8.cu -> libafqmc_ozaki.so (tcgen05 kind::i8 experiment) if missing or stale."""
+    srcs = [os.path.join(CSRC, "ozaki_i8.cu"), os.path.join(os.path.dirname(PKG_DIR), "include", "afqmc_ozaki.h")]
+    if not force and os.path.exists(OZAKI_LIB) and all(os.path.getmtime(s) <= os.path.getmtime(OZAKI_LIB) for s in srcs):
+        return OZAKI_LIB
+    cmd = [_nvcc(), *NVCC_FLAGS, "-o", OZAKI_LIB, srcs[0]]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
+    return OZAKI_LIB
 
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
@@ -23,10 +41,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         t = os.path.getmtime(LIB)
         if all(os.path.getmtime(s) <= t for s in _sources()):
             return LIB
-    nvcc = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
-    if not os.path.exists(nvcc):
-        nvcc = "nvcc"
-    cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, os.path.join(CSRC, "afqmc.cu")]
+    cmd = [_nvcc(), *NVCC_FLAGS, "-o", LIB, os.path.join(CSRC, "afqmc.cu")]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     res = subprocess.run(cmd, capture_output=True, text=True)
