@@ -40,6 +40,7 @@ struct SpinCfg {
     OperandLayout layA{}, layB{};
     double *A = nullptr, *B = nullptr, *psi = nullptr, *ht = nullptr, *tbuf = nullptr, *xpart = nullptr;
     double *psi_im = nullptr, *ht_im = nullptr;   // complex trial only
+    double *psiA = nullptr, *psiA_im = nullptr;   // psi^T as DMMA A fragments for K1's overlap product
     int nb = 0;                                   // rows of one gamma block of the A operand: n (real trial) or 2n
     bool cplx = false;                            // this spin's trial block has a non-zero imaginary part
     // dedicated force-bias path (afqmc_enable_force_bias): operands packed with n = 1, k = (i, p)
@@ -200,7 +201,7 @@ bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
     c.layB = OperandLayout{n, c.NT, ksteps, c.wT, (long long)c.NT * ksteps * 32};
     c.A_bytes = (size_t)c.n_rt * c.layA.tile_doubles * 8;
     c.B_bytes = (size_t)c.n_ct_max * c.layB.tile_doubles * 8;
-    c.k1_smem = (size_t)2 * n * n * 16 + (size_t)K1_PCHUNK * n * 16 + (size_t)2 * K1_PCHUNK * n * 8 + (size_t)n * 4 + 16;
+    c.k1_smem = (size_t)k1_layout(n, cplx).total;
     return true;
 }
 
@@ -244,6 +245,7 @@ void free_ctx(afqmc_ctx *c) {
     if (!c) return;
     for (int s = 0; s < 2; ++s) {
         cudaFree(c->sp[s].A); cudaFree(c->sp[s].B); cudaFree(c->sp[s].psi); cudaFree(c->sp[s].ht); cudaFree(c->sp[s].psi_im); cudaFree(c->sp[s].ht_im);
+        cudaFree(c->sp[s].psiA); cudaFree(c->sp[s].psiA_im);
         cudaFree(c->sp[s].f_A); cudaFree(c->sp[s].f_B); cudaFree(c->sp[s].f_craw);
         cudaFree(c->sp[s].tbuf); cudaFree(c->sp[s].xpart);
     }
@@ -278,24 +280,33 @@ int check_arch(afqmc_ctx *ctx, int *num_sms) {
     return AFQMC_OK;
 }
 
-// K1 for `n_walkers` walkers; with_fb also writes theta in the force-bias operand order.
-int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, cudaStream_t stream) {
+// K1 for `n_walkers` walkers; with_fb also writes theta in the force-bias operand order.  spin = -1: both spins in one
+// launch; 0 / 1: that spin only (the host-buffer entry point runs alpha while beta is still being copied).
+int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, cudaStream_t stream, int spin = -1) {
     const int N = ctx->N;
     K1Params p1{};
     p1.walkers = reinterpret_cast<const double2 *>(walkers);
     p1.n_walkers = n_walkers; p1.N = N; p1.maxw = ctx->maxw;
+    p1.spin0 = spin < 0 ? 0 : spin;
     p1.spin_off[0] = 0;
     p1.spin_off[1] = (long long)n_walkers * N * ctx->sp[0].n;
     for (int s = 0; s < 2; ++s) {
-        p1.n[s] = ctx->sp[s].n; p1.psi[s] = ctx->sp[s].psi; p1.ht[s] = ctx->sp[s].ht;
-        p1.psi_im[s] = ctx->sp[s].psi_im; p1.ht_im[s] = ctx->sp[s].ht_im;
+        p1.n[s] = ctx->sp[s].n; p1.psiA[s] = ctx->sp[s].psiA; p1.psiA_im[s] = ctx->sp[s].psiA_im;
+        p1.ht[s] = ctx->sp[s].ht; p1.ht_im[s] = ctx->sp[s].ht_im;
         p1.thetaB[s] = ctx->sp[s].B; p1.layB[s] = ctx->sp[s].layB;
         p1.thetaF[s] = with_fb ? ctx->sp[s].f_B : nullptr; p1.layF[s] = ctx->sp[s].f_layB;
     }
     p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
-    size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
-    if (with_fb) k1_overlap_inverse_theta<true><<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
-    else k1_overlap_inverse_theta<false><<<dim3(n_walkers, 2), K1_THREADS, k1s, stream>>>(p1);
+    const size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
+    const bool big = std::max(ctx->sp[0].n, ctx->sp[1].n) > 32;
+    const dim3 grid(n_walkers, spin < 0 ? 2 : 1);
+    if (big) {
+        if (with_fb) k1_overlap_inverse_theta<true, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
+        else k1_overlap_inverse_theta<true, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    } else {
+        if (with_fb) k1_overlap_inverse_theta<false, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
+        else k1_overlap_inverse_theta<false, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    }
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
     return AFQMC_OK;
@@ -420,6 +431,24 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
             CR_TRY(cudaMemcpyAsync(sc.psi_im, psi_ih.data(), psi_ih.size() * 8, cudaMemcpyHostToDevice, stream));
             CR_TRY(cudaMalloc(&sc.ht_im, (size_t)n * N * 8));
         }
+        {   // psi^T in DMMA A-fragment order for K1: [k-step][8-row strip of i][lane = r * 4 + k], p = 4 * kstep + k,
+            // zero-padded to whole chunks of K1_ROWS rows of phi (k1_overlap.cuh)
+            const int ns8 = (n + 7) / 8, kpad = 8 * ((N + K1_ROWS - 1) / K1_ROWS);
+            std::vector<double> pa((size_t)kpad * ns8 * 32, 0.0), pai(cplx ? pa.size() : 0, 0.0);
+            for (int p = 0; p < N; ++p)
+                for (int i = 0; i < n; ++i) {
+                    const size_t o = ((size_t)(p >> 2) * ns8 + (i >> 3)) * 32 + (i & 7) * 4 + (p & 3);
+                    pa[o] = psi_h[(size_t)p * n + i];
+                    if (cplx) pai[o] = psi_ih[(size_t)p * n + i];
+                }
+            CR_TRY(cudaMalloc(&sc.psiA, pa.size() * 8));
+            CR_TRY(cudaMemcpyAsync(sc.psiA, pa.data(), pa.size() * 8, cudaMemcpyHostToDevice, stream));
+            if (cplx) {
+                CR_TRY(cudaMalloc(&sc.psiA_im, pai.size() * 8));
+                CR_TRY(cudaMemcpyAsync(sc.psiA_im, pai.data(), pai.size() * 8, cudaMemcpyHostToDevice, stream));
+            }
+            CR_TRY(cudaStreamSynchronize(stream));
+        }
         CR_TRY(cudaStreamSynchronize(stream));
         CR_TRY(cudaMalloc(&sc.ht, (size_t)n * N * 8));
         CR_TRY(cudaMalloc(&sc.A, sc.A_bytes));
@@ -449,8 +478,10 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         }
         CR_TRY(allow_max_smem(fn));
     }
-    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<false>));
-    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<true>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<false, false>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<false, true>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<true, false>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<true, true>));
     CR_TRY(allow_max_smem(k5_spin_squared));
     CR_TRY(allow_max_smem(k6_greens_function));
     CR_TRY(cudaMalloc(&c->e1, (size_t)2 * max_walkers * 16));
