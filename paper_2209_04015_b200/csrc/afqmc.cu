@@ -1013,4 +1013,17 @@ int afqmc_fp64_peak(int mode, int launches, double *tflops, void *stream_) {
     return AFQMC_OK;
 }
 
+#ifdef AFQMC_K1_PHASE_CLOCKS
+// Diagnostic builds only (k1_overlap.cuh): out[0] = K1 CTAs run since the last call, out[1..7] = cycles from CTA start
+// to each phase boundary, summed over those CTAs.  Resets the counters.
+int afqmc_k1_phase_clocks(long long out[8]) {
+    if (!out) return AFQMC_ERR_ARG;
+    CU_TRY(nullptr, cudaDeviceSynchronize());
+    CU_TRY(nullptr, cudaMemcpyFromSymbol(out, afqmc::g_k1_clocks, 8 * sizeof(long long)));
+    const long long zero[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    CU_TRY(nullptr, cudaMemcpyToSymbol(afqmc::g_k1_clocks, zero, sizeof zero));
+    return AFQMC_OK;
+}
+#endif
+
 }  // extern "C"
