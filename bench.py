@@ -13,9 +13,10 @@ configuration BASELINE.json's metric is quoted on: Cu2O2-scale, N=290, n_alpha=n
              against the FP64 tensor (DMMA) peak measured live on this GPU with afqmc_fp64_peak
   cpu_baseline  the oracle (oracle/afqmc_oracle.py, rung O3) timed on this box's host cores on a bounded sample
 
-N > 1 (torchrun): the path shards over walkers with no data-path collective -- every rank owns Nw walkers of its
-own (weak scaling) and a replica of the half-rotated tensors; the only communication is the barrier and the
-max-over-ranks of the timings.
+N > 1: the path shards over walkers with no data-path collective -- the job has N * Nw walkers, rank r owns the r-th
+block of Nw (weak scaling) and a replica of the half-rotated tensors; the only communication is the barrier, the
+max-over-ranks of the timings and one gather of the per-walker energies for the result digest.  Launched under
+torchrun by the driver; a plain `python bench.py --gpus N` re-launches itself that way.
 
 --impl reference times the CPU oracle as it stands (rank 0 only) on a bounded sample per step.
 """
@@ -167,18 +168,28 @@ def main():
         run_reference(args, cfg, rank, world)
         return
 
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        # asked for N ranks from a plain `python bench.py --gpus N`: run the same command under torchrun
+        from paper_2209_04015_b200.parallel import respawn_under_torchrun
+        raise SystemExit(respawn_under_torchrun(os.path.abspath(__file__), args.gpus, sys.argv[1:]).returncode)
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU "
+                         f"(torchrun --nproc-per-node {args.gpus}) or drop --gpus")
+
     import torch
     import torch.distributed as dist
     from paper_2209_04015_b200 import LocalEnergy, fp64_peak_tflops
+    from paper_2209_04015_b200.parallel import (gather_walker_results, init_from_env, result_digest,
+                                                weak_scaling_block)
     from paper_2209_04015_b200.parallel import max_over_ranks as _max_over_ranks
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (this library has no CPU path)")
+    if torch.cuda.device_count() < world:
+        raise SystemExit(f"bench.py: {world} ranks but only {torch.cuda.device_count()} GPUs are visible")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+    init_from_env("nccl", dev)
 
     def barrier():
         if world > 1:
@@ -188,10 +199,13 @@ def main():
     def max_over_ranks(x):
         return _max_over_ranks(x, device=dev)
 
-    # ---- inputs: same Hamiltonian/trial on every rank, rank-specific walkers would come from the caller; here
-    # every rank evaluates the config's Nw walkers (weak scaling: per-GPU work fixed).
+    # ---- inputs: same Hamiltonian/trial on every rank; the job's population is world * Nw walkers of the config's
+    # generator (drawn walker by walker, so the first Nw are the one-rank job's) and rank r owns the r-th block.
     nw = cfg["n_walkers"]
-    inp = make_inputs(args.config)
+    w_start, w_count = weak_scaling_block(nw, rank, world)
+    assert w_count == nw
+    inp = make_inputs(args.config, n_walkers=world * nw)
+    my_walkers = list(range(w_start, w_start + w_count))
     h1e = torch.from_numpy(inp.h1e).to(dev)
     chol = torch.from_numpy(inp.chol).to(dev)
     trial = torch.from_numpy(inp.trial_packed()).to(dev)
@@ -203,7 +217,7 @@ def main():
         le.enable_propagation(h1e, chol, PROP_DT)
     del chol
     torch.cuda.empty_cache()
-    walkers_host = torch.from_numpy(inp.walkers_packed()).pin_memory()
+    walkers_host = torch.from_numpy(inp.walkers_packed(my_walkers)).pin_memory()
     walkers = walkers_host.to(dev)
     outE = torch.empty(nw, dtype=torch.complex128, device=dev)
     outO = torch.empty(nw, dtype=torch.complex128, device=dev)
@@ -214,8 +228,13 @@ def main():
     stream = torch.cuda.current_stream()
 
     # ---- FP64 peak, measured live (roofline denominator) ------------------------------------------------
+    psamp = ClockSampler(local_rank)
+    psamp.start()
     peak_dmma = fp64_peak_tflops("dmma", launches=20)
     peak_dfma = fp64_peak_tflops("dfma", launches=10)
+    peak_record = {"how": "afqmc_fp64_peak: register-resident chains, 20 back-to-back launches of mode 0 (DMMA.8x8x4, "
+                          "16 warps/SM x 8 accumulators) and 10 of mode 1 (DFMA), CUDA events around the sequence",
+                   "dmma_launches": 20, "dfma_launches": 10, "clocks": psamp.stop()}
 
     # ---- device-resident timing ---------------------------------------------------------------------------
     for _ in range(args.warmup):
@@ -251,6 +270,11 @@ def main():
     ms_e2e = max_over_ranks(e0.elapsed_time(e1))
     e2e_value = world * nw * args.steps / (ms_e2e * 1e-3)
     same = bool(torch.equal(outE_h.view(torch.float64), outE.cpu().view(torch.float64)))
+    # per-walker energies of the whole job in walker order: equal digests between an N-rank and a 1-rank run (its
+    # walkers are the first block) mean bit-identical results
+    all_E = gather_walker_results(outE, world * nw)
+    digest = {"first_block_sha256": result_digest(all_E[:nw]), "all_blocks_sha256": result_digest(all_E),
+              "n_walkers_total": world * nw}
 
     # ---- the force bias without the energy: K1 + one DMMA GEMM per spin + combine ------------------
     fb_out = torch.empty((nw, inp.n_gamma), dtype=torch.complex128, device=dev)
@@ -334,6 +358,9 @@ def main():
     t_roof_ms = max(flops_k2 / (peak * 1e12), bytes_l / (hbm_gbs * 1e9)) * 1e3
     roofline = {"bound": "tensor", "kernel": "k2_exchange (fused exchange + Coulomb traces), one launch per spin",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this "
+                                  "kernel, stored in profiles/k2_dram_traffic.json; not re-measured in this run",
+                "peak_measurement": peak_record,
                 "peak_source": "FP64 DMMA.8x8x4 register-resident microbenchmark (afqmc_fp64_peak) measured live in "
                                "this run; MEASURED_PEAKS.json has no FP64 entry",
                 "peak_dmma_tflops": peak_dmma, "peak_dfma_tflops": peak_dfma,
@@ -434,6 +461,7 @@ def main():
                         "d2h_bytes_per_step": int(2 * nw * 16), "ms_per_step": ms_e2e / args.steps,
                         "matches_device_path_bitwise": same},
                 "gpu_launches": int(gpu_launches),
+                "result_digest": digest,
                 "force_bias": {"value": world * nw / (ms_fb * 1e-3), "unit": UNIT, "ms_per_step": ms_fb,
                                "what": "afqmc_force_bias_only: K1 + [Ngamma x nN].[nN x 2Nw] DMMA GEMM per spin + "
                                        "combine; device-resident, same walkers",

@@ -36,6 +36,7 @@ struct SpinCfg {
     int n = 0;
     int MT = 0, NT = 0, WM = 0, gT = 0, wT = 0, strips = 0, ksc = 0, nchunks = 0, nstages = 0, H = 0, LD2 = 0;
     int n_rt = 0, n_ct_max = 0;
+    int ctas_per_sm = 1;                          // persistent K2 CTAs per SM (2: two half-size CTAs, epilogues overlap K loops)
     size_t k2_smem = 0, k1_smem = 0;
     OperandLayout layA{}, layB{};
     double *A = nullptr, *B = nullptr, *psi = nullptr, *ht = nullptr, *tbuf = nullptr, *xpart = nullptr;
@@ -64,6 +65,18 @@ const PipelineOverride &pipeline_override() {
     return ov;
 }
 
+// Tuning override AFQMC_K2_SHAPE="warps,ctas_per_sm,gT,wT" (benchmarks only): forces K2's CTA shape.
+struct ShapeOverride { bool set = false; int wm = 0, ctas = 0, gT = 0, wT = 0; };
+const ShapeOverride &shape_override() {
+    static const ShapeOverride ov = [] {
+        ShapeOverride o;
+        if (const char *e = std::getenv("AFQMC_K2_SHAPE"))
+            o.set = std::sscanf(e, "%d,%d,%d,%d", &o.wm, &o.ctas, &o.gT, &o.wT) == 4 && o.wm >= 1 && o.wm <= K2_MAX_WM && o.ctas >= 1 && o.ctas <= 4;
+        return o;
+    }();
+    return ov;
+}
+
 }  // namespace
 
 struct afqmc_ctx {
@@ -72,6 +85,8 @@ struct afqmc_ctx {
     SpinCfg sp[2];
     double *e1 = nullptr, *logdet = nullptr;
     double2 *h_walkers = nullptr;      // device staging for the host-buffer entry point
+    cudaStream_t copy_stream = nullptr; // carries the beta block's host-to-device copy under alpha's kernels
+    cudaEvent_t ev_alpha = nullptr, ev_beta = nullptr;
     double *h_outE = nullptr, *h_outO = nullptr;
     int last_nw = 0;                   // walkers whose theta the handle holds (last energy or force-bias-only call)
     int last_energy_nw = 0;            // walkers whose Coulomb traces the handle holds (last energy call)
@@ -131,10 +146,10 @@ size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages) {
 }
 
 // Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer.
-bool choose_pipeline(int strips, int NT, int ksteps, int &ksc, int &nst) {
+bool choose_pipeline(int strips, int NT, int ksteps, size_t budget, int &ksc, int &nst) {
     if (const PipelineOverride &ov = pipeline_override(); ov.set) {
         const int kc = ov.ksc, s = ov.stages;
-        if (kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 && k2_smem_bytes(strips, NT, kc, s) <= (size_t)kMaxSmem) {
+        if (kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 && k2_smem_bytes(strips, NT, kc, s) <= budget) {
             ksc = kc; nst = s;
             return true;
         }
@@ -145,7 +160,7 @@ bool choose_pipeline(int strips, int NT, int ksteps, int &ksc, int &nst) {
     for (int s = 2; s <= 5; ++s) {
         for (int kc = std::min(12, std::max(2, ksteps / 10)); kc >= 1; --kc) {   // short K loops want short chunks (tile start-up)
             if (kc > ksteps) continue;
-            if (k2_smem_bytes(strips, NT, kc, s) > (size_t)kMaxSmem) continue;
+            if (k2_smem_bytes(strips, NT, kc, s) > budget) continue;
             if (kc * s > best) { best = kc * s; ksc = kc; nst = s; }
             break;
         }
@@ -164,8 +179,12 @@ bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
     double best = -1.0;
     // Every warp of the CTA is an MMA warp: K2_MAX_WM = 12 warps (3 per SM sub-partition) is what the register file
     // allows at 168 registers per thread, and fewer warps never scored higher in any shape.
-    const int WM = K2_MAX_WM;
+    const ShapeOverride &so = shape_override();
+    const int WM = so.set ? so.wm : K2_MAX_WM;
+    c.ctas_per_sm = so.set ? so.ctas : 1;
+    const size_t budget = c.ctas_per_sm == 1 ? (size_t)kMaxSmem : (size_t)(233472 / c.ctas_per_sm - 1024);
     for (int wT = 1; wT <= K2_MAX_WT; ++wT) {
+        if (so.set && so.wT > 0 && wT != so.wT) continue;
         const int cols = 2 * wT * n, NT = (cols + 7) / 8;
         if (NT > 16) continue;
         const double colEff = cols / (8.0 * NT);
@@ -174,11 +193,12 @@ bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
             for (int gT = 1; gT <= n_gamma; ++gT) {
                 const int strips = (gT * nb + 7) / 8;
                 if (strips > MT * WM) break;
+                if (so.set && so.gT > 0 && gT != so.gT) continue;
                 if ((strips + WM - 1) / WM < MT && MT > 1) continue;   // a smaller MT covers it
                 const int maxload = (strips + 3) / 4;
                 const double rowEff = (gT * nb / 8.0) / (4.0 * maxload);
                 int ksc = 0, nst = 0;
-                if (!choose_pipeline(strips, NT, ksteps, ksc, nst)) continue;
+                if (!choose_pipeline(strips, NT, ksteps, budget, ksc, nst)) continue;
                 const long long ntiles = (long long)((n_gamma + gT - 1) / gT) * ((maxw + wT - 1) / wT);
                 const double fill = ntiles >= 148 ? 1.0 : ntiles / 148.0;
                 const double lds = 1.0 - 0.03 * (double)(MT + NT) / (MT * NT);
@@ -253,6 +273,9 @@ void free_ctx(afqmc_ctx *c) {
     cudaFree(c->hp); cudaFree(c->Emat); cudaFree(c->Etmp[0]); cudaFree(c->Etmp[1]); cudaFree(c->v_A); cudaFree(c->v_B);
     cudaFree(c->V); cudaFree(c->Vtri); cudaFree(c->fbuf); cudaFree(c->xbar); cudaFree(c->Tb[0]); cudaFree(c->Tb[1]); cudaFree(c->Tb[2]);
     cudaFree(c->lo_old); cudaFree(c->lo_new);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->ev_alpha) cudaEventDestroy(c->ev_alpha);
+    if (c->ev_beta) cudaEventDestroy(c->ev_beta);
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     for (auto &e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
@@ -489,6 +512,9 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
     CR_TRY(cudaMemsetAsync(c->e1, 0, (size_t)2 * max_walkers * 16, stream));
     CR_TRY(cudaMemsetAsync(c->logdet, 0, (size_t)2 * max_walkers * 16, stream));
     CR_TRY(cudaMalloc(&c->h_walkers, (size_t)max_walkers * N * (n_alpha + n_beta) * 16));
+    CR_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CR_TRY(cudaEventCreateWithFlags(&c->ev_alpha, cudaEventDisableTiming));
+    CR_TRY(cudaEventCreateWithFlags(&c->ev_beta, cudaEventDisableTiming));
     CR_TRY(cudaMalloc(&c->h_outE, (size_t)max_walkers * 16));
     CR_TRY(cudaMalloc(&c->h_outO, (size_t)max_walkers * 16));
     CR_TRY(cudaStreamSynchronize(stream));
@@ -497,25 +523,26 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
     return AFQMC_OK;
 }
 
-int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out_energies, void *out_overlaps,
-                       void *stream_) {
-    if (!ctx) return AFQMC_ERR_ARG;
-    if (!walkers || !out_energies || !out_overlaps) return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: null pointer argument");
-    if (n_walkers < 1 || n_walkers > ctx->maxw)
-        return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
-    cudaStream_t stream = (cudaStream_t)stream_;
-    const int N = ctx->N;
+// K1 -> K2 (once per spin) -> K3 on `stream`.  beta_ready != nullptr: the beta block of `walkers` is still being copied
+// on another stream, which records that event when it is done: alpha's K1 and K2 run first, beta's wait for the event.
+static int run_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out_energies, void *out_overlaps,
+                      cudaStream_t stream, cudaEvent_t beta_ready) {
     cudaEvent_t *ev = ctx->profiling ? &ctx->ev[(size_t)(ctx->prof_calls % kProfSets) * 4] : nullptr;
     if (ev) CU_TRY(ctx, cudaEventRecord(ev[0], stream));
+    const bool split = beta_ready != nullptr && ctx->sp[0].n > 0 && ctx->sp[1].n > 0;
 
-    // ---- K1 -------------------------------------------------------------------------------------------
-    if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream)) return rc;
+    // ---- K1 (both spins in one launch unless beta is still on its way) ------------------------------------
+    if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream, split ? 0 : -1)) return rc;
     if (ev) CU_TRY(ctx, cudaEventRecord(ev[1], stream));
 
     // ---- K2, once per spin ------------------------------------------------------------------------------
     for (int s = 0; s < 2; ++s) {
         const SpinCfg &sc = ctx->sp[s];
         if (sc.n == 0) continue;
+        if (split && s == 1) {
+            CU_TRY(ctx, cudaStreamWaitEvent(stream, beta_ready, 0));
+            if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream, 1)) return rc;
+        }
         K2Params p2{};
         p2.A = sc.A; p2.B = sc.B;
         p2.tileA_doubles = sc.layA.tile_doubles; p2.tileB_doubles = sc.layB.tile_doubles;
@@ -525,7 +552,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
         p2.n_gamma = ctx->n_gamma; p2.n_walkers = n_walkers; p2.maxw = ctx->maxw; p2.H = sc.H; p2.LD2 = sc.LD2;
         p2.tbuf = sc.tbuf; p2.xpart = sc.xpart;
         const long long ntiles = (long long)p2.n_rt * p2.n_ct;
-        const int grid = (int)std::min<long long>(ntiles, ctx->num_sms);
+        const int grid = (int)std::min<long long>(ntiles, (long long)ctx->num_sms * sc.ctas_per_sm);
         K2Fn fn = k2_pick(sc.MT, sc.NT);
         fn<<<grid, 32 * sc.WM, sc.k2_smem, stream>>>(p2);
         CU_TRY(ctx, cudaGetLastError());
@@ -551,6 +578,15 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     return AFQMC_OK;
 }
 
+int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out_energies, void *out_overlaps,
+                       void *stream_) {
+    if (!ctx) return AFQMC_ERR_ARG;
+    if (!walkers || !out_energies || !out_overlaps) return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: null pointer argument");
+    if (n_walkers < 1 || n_walkers > ctx->maxw)
+        return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
+    return run_energy(ctx, walkers, n_walkers, out_energies, out_overlaps, (cudaStream_t)stream_, nullptr);
+}
+
 int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walkers, void *out_energies_host,
                             void *out_overlaps_host, void *stream_) {
     if (!ctx) return AFQMC_ERR_ARG;
@@ -559,9 +595,20 @@ int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walk
     if (n_walkers < 1 || n_walkers > ctx->maxw)
         return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy_host: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
     cudaStream_t stream = (cudaStream_t)stream_;
-    const size_t wbytes = (size_t)n_walkers * ctx->N * (ctx->sp[0].n + ctx->sp[1].n) * 16;
-    CU_TRY(ctx, cudaMemcpyAsync(ctx->h_walkers, walkers_host, wbytes, cudaMemcpyHostToDevice, stream));
-    if (int rc = afqmc_local_energy(ctx, ctx->h_walkers, n_walkers, ctx->h_outE, ctx->h_outO, stream_)) return rc;
+    // The alpha block is copied on `stream`; the beta block follows it on the handle's copy stream and lands while
+    // alpha's K1 and K2 run (K2 of one spin is about half of the step, the copy of one block a few per cent of it).
+    const size_t a_bytes = (size_t)n_walkers * ctx->N * ctx->sp[0].n * 16, b_bytes = (size_t)n_walkers * ctx->N * ctx->sp[1].n * 16;
+    const bool split = a_bytes > 0 && b_bytes > 0;
+    const char *src = reinterpret_cast<const char *>(walkers_host);
+    char *dst = reinterpret_cast<char *>(ctx->h_walkers);
+    CU_TRY(ctx, cudaMemcpyAsync(dst, src, split ? a_bytes : a_bytes + b_bytes, cudaMemcpyHostToDevice, stream));
+    if (split) {
+        CU_TRY(ctx, cudaEventRecord(ctx->ev_alpha, stream));               // also orders the beta copy after earlier work on `stream`
+        CU_TRY(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_alpha, 0));
+        CU_TRY(ctx, cudaMemcpyAsync(dst + a_bytes, src + a_bytes, b_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
+        CU_TRY(ctx, cudaEventRecord(ctx->ev_beta, ctx->copy_stream));
+    }
+    if (int rc = run_energy(ctx, ctx->h_walkers, n_walkers, ctx->h_outE, ctx->h_outO, stream, split ? ctx->ev_beta : nullptr)) return rc;
     CU_TRY(ctx, cudaMemcpyAsync(out_energies_host, ctx->h_outE, (size_t)n_walkers * 16, cudaMemcpyDeviceToHost, stream));
     CU_TRY(ctx, cudaMemcpyAsync(out_overlaps_host, ctx->h_outO, (size_t)n_walkers * 16, cudaMemcpyDeviceToHost, stream));
     CU_TRY(ctx, cudaStreamSynchronize(stream));

@@ -8,8 +8,60 @@ the maximum of a timing over ranks.  Everything here works with any ``torch.dist
 """
 from __future__ import annotations
 
+import hashlib
+import os
+import socket
+import subprocess
+import sys
+
 import torch
 import torch.distributed as dist
+
+
+def torchrun_command(script: str, nproc: int, argv: list[str], port: int | None = None) -> list[str]:
+    """The command line that runs ``script argv`` as ``nproc`` ranks on this node (one process per GPU), the way
+    the benchmark driver launches it: ``python -m torch.distributed.run --nnodes=1 --nproc-per-node N ...``."""
+    if port is None:
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={nproc}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), script, *argv]
+
+
+def respawn_under_torchrun(script: str, nproc: int, argv: list[str], **popen_kw) -> subprocess.CompletedProcess:
+    """Re-run ``script`` as ``nproc`` ranks (used when a multi-rank run was asked for from a plain ``python`` call,
+    i.e. WORLD_SIZE is not set).  Returns the finished process; stdout/stderr pass through unless redirected."""
+    env = dict(os.environ)
+    env.pop("RANK", None)
+    env.pop("LOCAL_RANK", None)
+    return subprocess.run(torchrun_command(script, nproc, argv), env=env, **popen_kw)
+
+
+def init_from_env(backend: str, device=None) -> tuple[int, int, int]:
+    """(rank, world, local_rank) from the torchrun environment; initialises the process group when world > 1."""
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        if device is not None:
+            dist.init_process_group(backend, device_id=device)
+        else:
+            dist.init_process_group(backend)
+    return rank, world, local_rank
+
+
+def weak_scaling_block(walkers_per_rank: int, rank: int, world: int) -> tuple[int, int]:
+    """Weak scaling: the job has ``world * walkers_per_rank`` walkers and rank r owns the r-th block of them (the
+    ``walker_shard`` of the global population), so the first block is exactly the one-rank job's population."""
+    return walker_shard(world * walkers_per_rank, rank, world)
+
+
+def result_digest(values: torch.Tensor) -> str:
+    """SHA-256 of the raw bytes of per-walker complex128 results: equal digests mean bit-identical results."""
+    v = values.detach().to("cpu", torch.complex128).contiguous()
+    return hashlib.sha256(torch.view_as_real(v).numpy().tobytes()).hexdigest()
 
 
 def walker_shard(n_walkers: int, rank: int, world: int) -> tuple[int, int]:

@@ -77,3 +77,30 @@ def test_two_ranks_gather_equals_single_process(nw):
     E, lo = orc.local_energy_batch(inp, rung="O3")
     assert np.array_equal(Eg, np.asarray(E)) and np.array_equal(log, np.asarray(lo))
     assert tmax == 11.0
+
+
+def test_respawn_under_torchrun_runs_the_weak_scaling_protocol():
+    """`python bench.py --gpus N` without torchrun re-launches itself with parallel.respawn_under_torchrun; here the
+    same helper starts tests/multirank_worker.py as 2 gloo ranks.  The first block's digest must equal the one-rank
+    run's (bit-identical energies), and the whole job's digest the single-process evaluation of all walkers."""
+    import json
+    import subprocess
+    import sys
+    from paper_2209_04015_b200.parallel import respawn_under_torchrun, result_digest, torchrun_command, weak_scaling_block
+    from gen import make_inputs
+    from oracle import afqmc_oracle as orc
+    worker = os.path.join(os.path.dirname(os.path.abspath(__file__)), "multirank_worker.py")
+    cmd = torchrun_command(worker, 2, ["3"], port=1234)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=2" in cmd and "127.0.0.1" in cmd
+    assert weak_scaling_block(3, 1, 2) == (3, 3)
+    two = respawn_under_torchrun(worker, 2, ["3"], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, timeout=600)
+    assert two.returncode == 0, two.stderr[-2000:]
+    r2 = json.loads([ln for ln in two.stdout.splitlines() if ln.startswith("{")][-1])
+    one = subprocess.run([sys.executable, worker, "3"], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, timeout=600,
+                         env={k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")})
+    assert one.returncode == 0, one.stderr[-2000:]
+    r1 = json.loads([ln for ln in one.stdout.splitlines() if ln.startswith("{")][-1])
+    assert r2["world"] == 2 and r1["world"] == 1 and r2["tmax"] == 11.0
+    assert r2["first_block_sha256"] == r1["first_block_sha256"] == r1["all_blocks_sha256"]
+    E, _ = orc.local_energy_batch(make_inputs("tiny", n_walkers=6), rung="O3")
+    assert r2["all_blocks_sha256"] == result_digest(torch.from_numpy(np.asarray(E, dtype=np.complex128)))
