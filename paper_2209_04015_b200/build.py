@@ -36,12 +36,14 @@ def build_ozaki_library(force: bool = False) -> str:
 
 
 def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/afqmc.cu -> libafqmc.so if missing or older than any source.  Returns the path."""
+    """Compile csrc/afqmc.cu -> libafqmc.so if missing or older than any source.  Returns the path.
+    AFQMC_NVCC_EXTRA adds compiler flags for diagnostic builds (-DAFQMC_K1_PHASE_CLOCKS, -DAFQMC_K2_ABLATE=n: see the
+    kernels' headers); such a build must be forced and must be replaced by a plain one afterwards."""
     if not force and os.path.exists(LIB):
         t = os.path.getmtime(LIB)
         if all(os.path.getmtime(s) <= t for s in _sources()):
             return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS, "-o", LIB, os.path.join(CSRC, "afqmc.cu")]
+    cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("AFQMC_NVCC_EXTRA", "").split(), "-o", LIB, os.path.join(CSRC, "afqmc.cu")]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     res = subprocess.run(cmd, capture_output=True, text=True)

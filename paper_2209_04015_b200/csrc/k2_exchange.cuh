@@ -18,6 +18,14 @@
 #include <type_traits>
 #include "common.cuh"
 
+// Timing ablations (results are WRONG, only the time is meaningful; never define this in a product build; build.py passes
+// AFQMC_NVCC_EXTRA through):  -DAFQMC_K2_ABLATE=1  epilogue parks the accumulators but skips phase 2 (the T_ij T_ji sums);
+// =2  no epilogue at all (K loop only);  =3  K loop without the ring's full / empty barriers and without the producer
+// (the operands are whatever the shared memory holds) and no epilogue.  profiles/r2_k2_ablations.md has the numbers.
+#ifndef AFQMC_K2_ABLATE
+#define AFQMC_K2_ABLATE 0
+#endif
+
 namespace afqmc {
 
 constexpr int K2_MAX_WT = 4;       // walkers per CTA tile
@@ -105,11 +113,13 @@ __device__ __forceinline__ void k2_tile_mma(double (&acc)[MM][NT][2], K2Ring &R,
 #pragma unroll 1
     for (int c = 0; c < R.nchunks; ++c) {
         const int nks = (c == R.nchunks - 1) ? R.last_ks : R.ksc;
+#if AFQMC_K2_ABLATE != 3
         if (producer_warp) {                       // refill at most one released stage per chunk, never blocking
             if (lane == 0) produce_poll();
             __syncwarp();
         }
         k2_wait_full(R.full_bar + 8u * R.stage, R.phase, producer_warp, lane, produce_poll);
+#endif
         uint32_t pa = R.smem_base + R.stage * R.stage_bytes + frag_off;          // + warp * 256 + lane * 8 (in frag_off)
         uint32_t pb = R.smem_base + R.stage * R.stage_bytes + R.a_chunk_bytes + 8u * lane;
 #pragma unroll 1
@@ -126,8 +136,10 @@ __device__ __forceinline__ void k2_tile_mma(double (&acc)[MM][NT][2], K2Ring &R,
             pa += R.a_kstride;
             pb += NT * 256u;
         }
+#if AFQMC_K2_ABLATE != 3
         __syncwarp();
         if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(R.empty_bar + 8u * R.stage) : "memory");
+#endif
         if (++R.stage == R.nstages) { R.stage = 0; R.phase ^= 1u; }
     }
 }
@@ -236,6 +248,7 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
             //     element (row, col)  ->  (row >> 1) * LD2 + (row & 1) * H + col,     H = 8 mod 16,  LD2 = 1 mod 16,
             // which makes the fragment-order stores here, the row loads and the column loads of phase 2 all
             // bank-conflict free (column loads 2-way when g*n is odd).
+#if AFQMC_K2_ABLATE < 2
             mbar_wait(stg_free, tpar ^ 1u);                                    // previous tile has been read out
             if constexpr (MM > 0) {
 #pragma unroll
@@ -265,7 +278,11 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
                 double *redp = red + tpar * (K2_MAX_WT * K2_MAX_WM * 2);      // double-buffered by tile parity
                 if (lane < K2_MAX_WT) { redp[(lane * K2_MAX_WM + warp) * 2] = 0.0; redp[(lane * K2_MAX_WM + warp) * 2 + 1] = 0.0; }
                 mbar_wait(stg_full, tpar);
+#if AFQMC_K2_ABLATE == 1
+                for (int u = warp; u < 0; u += WM) {
+#else
                 for (int u = warp; u < nblk * rs; u += WM) {
+#endif
                     const int blk = u / rs, part = u - blk * rs;
                     const int g = blk / wvalid, wl = blk - g * wvalid;
                     const int i_lo = (part * n) / rs, i_hi = ((part + 1) * n) / rs;
@@ -330,6 +347,16 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
                     }
                 }
             }
+#else   // keep the products alive (ptxas would drop DMMAs whose results are never read)
+            if constexpr (MM > 0) {
+                double keep = 0.0;
+#pragma unroll
+                for (int m = 0; m < MM; ++m)
+#pragma unroll
+                    for (int q = 0; q < NT; ++q) keep += acc[m][q][0] + acc[m][q][1];
+                if (keep == 1.2345678e300) P.tbuf[0] = keep;
+            }
+#endif  // AFQMC_K2_ABLATE < 2
             tpar ^= 1u;
             rt += step_rt; ct += step_ct;
             if (ct >= P.n_ct) { ct -= P.n_ct; ++rt; }
