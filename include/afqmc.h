@@ -89,9 +89,10 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
 /*
  * afqmc_local_energy_host -- the same computation with HOST buffers: copies `walkers_host` to an internal
  * device buffer, runs the kernels, copies both outputs back, and synchronises `stream` before returning.  Layouts as
- * above.  The alpha block is copied on `stream`, the beta block right behind it on a stream of the handle's own, so
- * that it lands while alpha's K1 and K2 run (K1 is launched once per spin here; results are bit-identical to
- * afqmc_local_energy).  Pinned host memory makes the copies asynchronous DMA; with pageable memory they serialise.
+ * above.  The walkers travel in three blocks -- the first eighth of the alpha block on `stream`, then the rest of it and
+ * the beta block on a stream of the handle's own -- and K1 + K2 run block by block, so that all but the first copy land
+ * under the kernels (results are bit-identical to afqmc_local_energy: the blocks are whole K2 column tiles).  Pinned host
+ * memory makes the copies asynchronous DMA; with pageable memory they serialise.
  */
 int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walkers, void *out_energies_host,
                             void *out_overlaps_host, void *stream);

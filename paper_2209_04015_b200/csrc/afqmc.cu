@@ -86,7 +86,7 @@ struct afqmc_ctx {
     double *e1 = nullptr, *logdet = nullptr;
     double2 *h_walkers = nullptr;      // device staging for the host-buffer entry point
     cudaStream_t copy_stream = nullptr; // carries the beta block's host-to-device copy under alpha's kernels
-    cudaEvent_t ev_alpha = nullptr, ev_beta = nullptr;
+    cudaEvent_t ev_first = nullptr, ev_rest = nullptr, ev_beta = nullptr;
     double *h_outE = nullptr, *h_outO = nullptr;
     int last_nw = 0;                   // walkers whose theta the handle holds (last energy or force-bias-only call)
     int last_energy_nw = 0;            // walkers whose Coulomb traces the handle holds (last energy call)
@@ -274,7 +274,8 @@ void free_ctx(afqmc_ctx *c) {
     cudaFree(c->V); cudaFree(c->Vtri); cudaFree(c->fbuf); cudaFree(c->xbar); cudaFree(c->Tb[0]); cudaFree(c->Tb[1]); cudaFree(c->Tb[2]);
     cudaFree(c->lo_old); cudaFree(c->lo_new);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
-    if (c->ev_alpha) cudaEventDestroy(c->ev_alpha);
+    if (c->ev_first) cudaEventDestroy(c->ev_first);
+    if (c->ev_rest) cudaEventDestroy(c->ev_rest);
     if (c->ev_beta) cudaEventDestroy(c->ev_beta);
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     for (auto &e : c->ev) if (e) cudaEventDestroy(e);
@@ -304,13 +305,16 @@ int check_arch(afqmc_ctx *ctx, int *num_sms) {
 }
 
 // K1 for `n_walkers` walkers; with_fb also writes theta in the force-bias operand order.  spin = -1: both spins in one
-// launch; 0 / 1: that spin only (the host-buffer entry point runs alpha while beta is still being copied).
-int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, cudaStream_t stream, int spin = -1) {
+// launch; 0 / 1: that spin only, walkers w0 .. w0 + count - 1 (the host-buffer entry point starts on the walkers that
+// have arrived while the rest is still being copied).  n_walkers is always the call's total (it fixes the beta offset).
+int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, cudaStream_t stream, int spin = -1, int w0 = 0,
+              int count = -1) {
     const int N = ctx->N;
     K1Params p1{};
     p1.walkers = reinterpret_cast<const double2 *>(walkers);
     p1.n_walkers = n_walkers; p1.N = N; p1.maxw = ctx->maxw;
     p1.spin0 = spin < 0 ? 0 : spin;
+    p1.w0 = w0;
     p1.spin_off[0] = 0;
     p1.spin_off[1] = (long long)n_walkers * N * ctx->sp[0].n;
     for (int s = 0; s < 2; ++s) {
@@ -322,7 +326,7 @@ int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, 
     p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
     const size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
     const bool big = std::max(ctx->sp[0].n, ctx->sp[1].n) > 32;
-    const dim3 grid(n_walkers, spin < 0 ? 2 : 1);
+    const dim3 grid(count < 0 ? n_walkers : count, spin < 0 ? 2 : 1);
     if (big) {
         if (with_fb) k1_overlap_inverse_theta<true, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
         else k1_overlap_inverse_theta<true, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
@@ -513,7 +517,8 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
     CR_TRY(cudaMemsetAsync(c->logdet, 0, (size_t)2 * max_walkers * 16, stream));
     CR_TRY(cudaMalloc(&c->h_walkers, (size_t)max_walkers * N * (n_alpha + n_beta) * 16));
     CR_TRY(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-    CR_TRY(cudaEventCreateWithFlags(&c->ev_alpha, cudaEventDisableTiming));
+    CR_TRY(cudaEventCreateWithFlags(&c->ev_first, cudaEventDisableTiming));
+    CR_TRY(cudaEventCreateWithFlags(&c->ev_rest, cudaEventDisableTiming));
     CR_TRY(cudaEventCreateWithFlags(&c->ev_beta, cudaEventDisableTiming));
     CR_TRY(cudaMalloc(&c->h_outE, (size_t)max_walkers * 16));
     CR_TRY(cudaMalloc(&c->h_outO, (size_t)max_walkers * 16));
@@ -523,40 +528,49 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
     return AFQMC_OK;
 }
 
-// K1 -> K2 (once per spin) -> K3 on `stream`.  beta_ready != nullptr: the beta block of `walkers` is still being copied
-// on another stream, which records that event when it is done: alpha's K1 and K2 run first, beta's wait for the event.
+// One K2 launch: spin s, walkers w0 .. w0 + count - 1 (w0 a multiple of the tile's walker count).
+static int launch_k2(afqmc_ctx *ctx, int s, int w0, int count, cudaStream_t stream) {
+    const SpinCfg &sc = ctx->sp[s];
+    K2Params p2{};
+    p2.A = sc.A; p2.B = sc.B + (long long)(w0 / sc.wT) * sc.layB.tile_doubles;
+    p2.tileA_doubles = sc.layA.tile_doubles; p2.tileB_doubles = sc.layB.tile_doubles;
+    p2.n = sc.n; p2.nb = sc.nb; p2.cplx = sc.cplx ? 1 : 0; p2.gT = sc.gT; p2.wT = sc.wT; p2.strips = sc.strips; p2.WM = sc.WM;
+    p2.ksteps = ctx->ksteps; p2.ksc = sc.ksc; p2.nchunks = sc.nchunks; p2.nstages = sc.nstages;
+    p2.n_rt = sc.n_rt; p2.n_ct = (count + sc.wT - 1) / sc.wT;
+    p2.n_gamma = ctx->n_gamma; p2.n_walkers = count; p2.maxw = ctx->maxw; p2.H = sc.H; p2.LD2 = sc.LD2;
+    p2.tbuf = sc.tbuf + (long long)w0 * ctx->n_gamma * 2; p2.xpart = sc.xpart + (long long)w0 * 2;
+    const long long ntiles = (long long)p2.n_rt * p2.n_ct;
+    const int grid = (int)std::min<long long>(ntiles, (long long)ctx->num_sms * sc.ctas_per_sm);
+    K2Fn fn = k2_pick(sc.MT, sc.NT);
+    fn<<<grid, 32 * sc.WM, sc.k2_smem, stream>>>(p2);
+    CU_TRY(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    return AFQMC_OK;
+}
+
+// A piece of an energy call: K1 and K2 of one spin on a range of walkers, after an optional event (the host-buffer entry
+// point records one per block of walkers it copies on its own stream).
+struct EnergyPiece { int spin, w0, count; cudaEvent_t wait; };
+
+// K1 -> K2 -> K3 on `stream`.  Without pieces: K1 for both spins in one launch, then K2 once per spin.
 static int run_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void *out_energies, void *out_overlaps,
-                      cudaStream_t stream, cudaEvent_t beta_ready) {
+                      cudaStream_t stream, const EnergyPiece *pieces, int n_pieces) {
     cudaEvent_t *ev = ctx->profiling ? &ctx->ev[(size_t)(ctx->prof_calls % kProfSets) * 4] : nullptr;
     if (ev) CU_TRY(ctx, cudaEventRecord(ev[0], stream));
-    const bool split = beta_ready != nullptr && ctx->sp[0].n > 0 && ctx->sp[1].n > 0;
-
-    // ---- K1 (both spins in one launch unless beta is still on its way) ------------------------------------
-    if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream, split ? 0 : -1)) return rc;
-    if (ev) CU_TRY(ctx, cudaEventRecord(ev[1], stream));
-
-    // ---- K2, once per spin ------------------------------------------------------------------------------
-    for (int s = 0; s < 2; ++s) {
-        const SpinCfg &sc = ctx->sp[s];
-        if (sc.n == 0) continue;
-        if (split && s == 1) {
-            CU_TRY(ctx, cudaStreamWaitEvent(stream, beta_ready, 0));
-            if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream, 1)) return rc;
+    if (n_pieces == 0) {
+        if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream)) return rc;
+        if (ev) CU_TRY(ctx, cudaEventRecord(ev[1], stream));
+        for (int s = 0; s < 2; ++s)
+            if (ctx->sp[s].n > 0)
+                if (int rc = launch_k2(ctx, s, 0, n_walkers, stream)) return rc;
+    } else {
+        for (int k = 0; k < n_pieces; ++k) {
+            const EnergyPiece &pc = pieces[k];
+            if (pc.wait) CU_TRY(ctx, cudaStreamWaitEvent(stream, pc.wait, 0));
+            if (int rc = launch_k1(ctx, walkers, n_walkers, false, stream, pc.spin, pc.w0, pc.count)) return rc;
+            if (ev && k == 0) CU_TRY(ctx, cudaEventRecord(ev[1], stream));
+            if (int rc = launch_k2(ctx, pc.spin, pc.w0, pc.count, stream)) return rc;
         }
-        K2Params p2{};
-        p2.A = sc.A; p2.B = sc.B;
-        p2.tileA_doubles = sc.layA.tile_doubles; p2.tileB_doubles = sc.layB.tile_doubles;
-        p2.n = sc.n; p2.nb = sc.nb; p2.cplx = sc.cplx ? 1 : 0; p2.gT = sc.gT; p2.wT = sc.wT; p2.strips = sc.strips; p2.WM = sc.WM;
-        p2.ksteps = ctx->ksteps; p2.ksc = sc.ksc; p2.nchunks = sc.nchunks; p2.nstages = sc.nstages;
-        p2.n_rt = sc.n_rt; p2.n_ct = (n_walkers + sc.wT - 1) / sc.wT;
-        p2.n_gamma = ctx->n_gamma; p2.n_walkers = n_walkers; p2.maxw = ctx->maxw; p2.H = sc.H; p2.LD2 = sc.LD2;
-        p2.tbuf = sc.tbuf; p2.xpart = sc.xpart;
-        const long long ntiles = (long long)p2.n_rt * p2.n_ct;
-        const int grid = (int)std::min<long long>(ntiles, (long long)ctx->num_sms * sc.ctas_per_sm);
-        K2Fn fn = k2_pick(sc.MT, sc.NT);
-        fn<<<grid, 32 * sc.WM, sc.k2_smem, stream>>>(p2);
-        CU_TRY(ctx, cudaGetLastError());
-        ctx->launches += 1;
     }
     if (ev) CU_TRY(ctx, cudaEventRecord(ev[2], stream));
 
@@ -584,7 +598,7 @@ int afqmc_local_energy(afqmc_ctx *ctx, const void *walkers, int n_walkers, void 
     if (!walkers || !out_energies || !out_overlaps) return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: null pointer argument");
     if (n_walkers < 1 || n_walkers > ctx->maxw)
         return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
-    return run_energy(ctx, walkers, n_walkers, out_energies, out_overlaps, (cudaStream_t)stream_, nullptr);
+    return run_energy(ctx, walkers, n_walkers, out_energies, out_overlaps, (cudaStream_t)stream_, nullptr, 0);
 }
 
 int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walkers, void *out_energies_host,
@@ -595,20 +609,37 @@ int afqmc_local_energy_host(afqmc_ctx *ctx, const void *walkers_host, int n_walk
     if (n_walkers < 1 || n_walkers > ctx->maxw)
         return fail(ctx, AFQMC_ERR_ARG, "afqmc_local_energy_host: n_walkers=%d outside 1..%d", n_walkers, ctx->maxw);
     cudaStream_t stream = (cudaStream_t)stream_;
-    // The alpha block is copied on `stream`; the beta block follows it on the handle's copy stream and lands while
-    // alpha's K1 and K2 run (K2 of one spin is about half of the step, the copy of one block a few per cent of it).
-    const size_t a_bytes = (size_t)n_walkers * ctx->N * ctx->sp[0].n * 16, b_bytes = (size_t)n_walkers * ctx->N * ctx->sp[1].n * 16;
-    const bool split = a_bytes > 0 && b_bytes > 0;
+    // Blocks of walkers are copied in the order the kernels want them: the first eighth of the first spin on `stream`,
+    // then -- on the handle's copy stream, one event each -- the rest of that spin and the other spin.  K1 + K2 start on
+    // the first block while the others land under them (K2 on an eighth of one spin takes several times longer than the
+    // copy of everything that is left); only the first block's copy is exposed.
+    const int N = ctx->N, na = ctx->sp[0].n, nb = ctx->sp[1].n;
     const char *src = reinterpret_cast<const char *>(walkers_host);
     char *dst = reinterpret_cast<char *>(ctx->h_walkers);
-    CU_TRY(ctx, cudaMemcpyAsync(dst, src, split ? a_bytes : a_bytes + b_bytes, cudaMemcpyHostToDevice, stream));
-    if (split) {
-        CU_TRY(ctx, cudaEventRecord(ctx->ev_alpha, stream));               // also orders the beta copy after earlier work on `stream`
-        CU_TRY(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_alpha, 0));
+    const size_t a_bytes = (size_t)n_walkers * N * na * 16, b_bytes = (size_t)n_walkers * N * nb * 16;
+    EnergyPiece pieces[3];
+    int n_pieces = 0;
+    const int s0 = na > 0 ? 0 : 1;                                        // first spin with electrons
+    const size_t off0 = s0 == 0 ? 0 : a_bytes, row_bytes = (size_t)N * ctx->sp[s0].n * 16;
+    const int wT = ctx->sp[s0].wT;
+    int first = ((n_walkers + 7) / 8 + wT - 1) / wT * wT;               // an eighth, in whole K2 column tiles
+    if (first >= n_walkers || n_walkers < 16 * wT) first = n_walkers;    // small batches: one block per spin
+    CU_TRY(ctx, cudaMemcpyAsync(dst + off0, src + off0, first * row_bytes, cudaMemcpyHostToDevice, stream));
+    CU_TRY(ctx, cudaEventRecord(ctx->ev_first, stream));                   // also orders the other copies after earlier work on `stream`
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_first, 0));
+    pieces[n_pieces++] = EnergyPiece{s0, 0, first, nullptr};
+    if (first < n_walkers) {
+        CU_TRY(ctx, cudaMemcpyAsync(dst + off0 + first * row_bytes, src + off0 + first * row_bytes, (n_walkers - first) * row_bytes,
+                                    cudaMemcpyHostToDevice, ctx->copy_stream));
+        CU_TRY(ctx, cudaEventRecord(ctx->ev_rest, ctx->copy_stream));
+        pieces[n_pieces++] = EnergyPiece{s0, first, n_walkers - first, ctx->ev_rest};
+    }
+    if (s0 == 0 && nb > 0) {
         CU_TRY(ctx, cudaMemcpyAsync(dst + a_bytes, src + a_bytes, b_bytes, cudaMemcpyHostToDevice, ctx->copy_stream));
         CU_TRY(ctx, cudaEventRecord(ctx->ev_beta, ctx->copy_stream));
+        pieces[n_pieces++] = EnergyPiece{1, 0, n_walkers, ctx->ev_beta};
     }
-    if (int rc = run_energy(ctx, ctx->h_walkers, n_walkers, ctx->h_outE, ctx->h_outO, stream, split ? ctx->ev_beta : nullptr)) return rc;
+    if (int rc = run_energy(ctx, ctx->h_walkers, n_walkers, ctx->h_outE, ctx->h_outO, stream, pieces, n_pieces)) return rc;
     CU_TRY(ctx, cudaMemcpyAsync(out_energies_host, ctx->h_outE, (size_t)n_walkers * 16, cudaMemcpyDeviceToHost, stream));
     CU_TRY(ctx, cudaMemcpyAsync(out_overlaps_host, ctx->h_outO, (size_t)n_walkers * 16, cudaMemcpyDeviceToHost, stream));
     CU_TRY(ctx, cudaStreamSynchronize(stream));

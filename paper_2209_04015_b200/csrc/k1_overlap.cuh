@@ -27,6 +27,7 @@ struct K1Params {
     const double2 *walkers;       // alpha block [Nw][N][na], then beta block [Nw][N][nb]
     int n_walkers, N, maxw;
     int spin0;                    // spin of blockIdx.y == 0 (per-spin launches of the host-buffer entry point)
+    int w0;                       // walker of blockIdx.x == 0 (launches on a range of walkers)
     int n[2];
     long long spin_off[2];        // offset of each spin block in `walkers`, in complex elements
     const double *psiA[2];        // Re psi^T as DMMA A fragments: [8 * chunks][strips][32], zero-padded
@@ -245,7 +246,7 @@ template <bool BIG, bool WITH_FB>
 __global__ void __launch_bounds__(K1_THREADS, BIG ? 1 : 4) k1_overlap_inverse_theta(K1Params P) {
     constexpr int MAXT_S = BIG ? 16 : 4;     // S pass: tiles per warp
     constexpr int MAXT_T = BIG ? 8 : 4;      // theta pass: column blocks per warp
-    const int w = blockIdx.x, sp = blockIdx.y + P.spin0;
+    const int w = blockIdx.x + P.w0, sp = blockIdx.y + P.spin0;
     const int n = P.n[sp], N = P.N;
     if (n == 0) return;
 #ifdef AFQMC_K1_PHASE_CLOCKS
