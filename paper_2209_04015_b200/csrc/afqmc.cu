@@ -324,9 +324,10 @@ int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, 
         p1.thetaF[s] = with_fb ? ctx->sp[s].f_B : nullptr; p1.layF[s] = ctx->sp[s].f_layB;
     }
     p1.logdet = ctx->logdet; p1.e1 = ctx->e1;
-    const size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
     const bool big = std::max(ctx->sp[0].n, ctx->sp[1].n) > 32;
-    const dim3 grid(count < 0 ? n_walkers : count, spin < 0 ? 2 : 1);
+    const int nwl = count < 0 ? n_walkers : count, nsp = spin < 0 ? 2 : 1;
+    const size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
+    const dim3 grid(nwl, nsp);
     if (big) {
         if (with_fb) k1_overlap_inverse_theta<true, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
         else k1_overlap_inverse_theta<true, false><<<grid, K1_THREADS, k1s, stream>>>(p1);

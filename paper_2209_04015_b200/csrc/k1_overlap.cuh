@@ -142,8 +142,8 @@ __device__ __noinline__ K1SlowPivot k1_slow_pivot(uint32_t cur, int n, int k, un
     return K1SlowPivot{inv.x, inv.y, r};
 }
 
-// X = S^-1 by n exchange steps (Gauss-Jordan, partial pivoting without row swaps), all 256 threads, one CTA barrier per
-// step.  Step k with pivot row r (the unused row of largest |a_rk|), p = a_rk, q_j = a_rj / p (j != k), q_k = -1/p:
+// X = S^-1 by n exchange steps (Gauss-Jordan, partial pivoting without row swaps), all THREADS threads of the CTA, one
+// CTA barrier per step.  Step k with pivot row r (the unused row of largest |a_rk|), p = a_rk, q_j = a_rj / p (j != k), q_k = -1/p:
 //     a_rj <- -q_j,        a_ij <- a_ij - a_ik q_j   (i != r; with a_ik taken as 0 on the left for j = k)
 // i.e. a_rk <- 1/p, a_rj <- -a_rj/p, a_ik <- a_ik/p, a_ij <- a_ij - a_ik a_rj/p.  Afterwards X_ij = W[rowof[i]][kof[j]]
 // and det S = sgn(k -> rowof[k]) prod_k p_k.  The matrix ping-pongs between w_start and w_other (shared-window addresses,
@@ -155,10 +155,10 @@ __device__ __noinline__ K1SlowPivot k1_slow_pivot(uint32_t cur, int n, int k, un
 // rows and take the maximum of the bit patterns with three warp-wide integer reductions.
 // Returns false if S is singular (a column is exactly zero below the used rows).  Not inlined: the loop then has the
 // kernel's whole register budget to itself (the caller's live values are parked on the stack once, outside the loop).
-template <int ROWS, int LG>
+template <int ROWS, int LG, int THREADS>
 __device__ __noinline__ bool k1_gauss_jordan(const int n, const uint32_t w_start, const uint32_t w_other, const uint32_t keys_u,
                                                 int *rowof, double2 *pivs, const int tid) {
-    constexpr int RY = K1_THREADS >> LG;
+    constexpr int RY = THREADS >> LG;
     const int lane = tid & 31, tx = tid & ((1 << LG) - 1), ty = tid >> LG;
     const bool col_ok = tx < n;
     const uint32_t txo = (col_ok ? tx : 0) * 16u;
@@ -223,6 +223,69 @@ __device__ __noinline__ bool k1_gauss_jordan(const int n, const uint32_t w_start
         const uint32_t t = cur; cur = nxt; nxt = t;
     }
     return true;
+}
+
+// ---- K loops of the two products --------------------------------------------------------------------------------------
+// A predicated-off DMMA still occupies the tensor pipe for its 16 cycles (measured: a kernel whose complex-trial DMMAs
+// were compiled as @!P DMMA ran its S pass at twice the pipe time), so nothing in these loops is predicated: the number
+// of column blocks a warp owns (CNT) and the complex-trial second product (CPLX) are template parameters, dispatched
+// once per chunk by a warp-uniform branch.
+
+// S pass, one chunk: nks k-steps.  pa: psi fragment of this warp's strip (+ im_off: Im psi), pb: B fragment of its first
+// column block in the staged rows of phi, a_step / b_step: bytes per k-step.
+template <int MAXT, int CNT, bool CPLX>
+__device__ __forceinline__ void k1_s_kloop(double (&acc)[MAXT][2], uint32_t pa, uint32_t pb, const int nks, const uint32_t a_step,
+                                           const uint32_t b_step, const uint32_t im_off, const bool odd_col) {
+    for (int ks = 0; ks < nks; ++ks) {
+        const double a = lds_f64_dyn(pa);
+        double a2 = 0.0;
+        if constexpr (CPLX) a2 = lds_f64_dyn(pa + im_off);
+#pragma unroll
+        for (int q = 0; q < CNT; ++q) {
+            const double b = lds_f64_dyn(pb + q * 64);
+            dmma_m8n8k4(acc[q][0], acc[q][1], a, b);
+            if constexpr (CPLX) {     // + Im psi^T (phi_im, -phi_re): (a - ib)(x + iy) = (ax + by) + i(ay - bx)
+                const double sw = lds_f64_dyn((pb + q * 64) ^ 8u);       // the other component of the same element
+                dmma_m8n8k4(acc[q][0], acc[q][1], a2, odd_col ? -sw : sw);
+            }
+        }
+        pa += a_step;
+        pb += b_step;
+    }
+}
+template <int MAXT, int CNT, bool CPLX>
+__device__ __forceinline__ void k1_s_dispatch(const int cnt, double (&acc)[MAXT][2], uint32_t pa, uint32_t pb, const int nks,
+                                              const uint32_t a_step, const uint32_t b_step, const uint32_t im_off, const bool odd_col) {
+    if constexpr (CNT > 0) {
+        if (cnt == CNT) k1_s_kloop<MAXT, CNT, CPLX>(acc, pa, pb, nks, a_step, b_step, im_off, odd_col);
+        else k1_s_dispatch<MAXT, CNT - 1, CPLX>(cnt, acc, pa, pb, nks, a_step, b_step, im_off, odd_col);
+    }
+}
+
+// theta pass, one chunk of one strip: kth k-steps.  pa: A fragment in the staged rows of phi, pb: this lane's component
+// of the first column block's XF entry, b_step: bytes of XF per k-step, flip: sign-bit mask of the (re column, im row) lanes.
+template <int MAXT, int CNT>
+__device__ __forceinline__ void k1_t_kloop(double (&acc)[MAXT][2], uint32_t pa, uint32_t pb, const int kth, const uint32_t b_step,
+                                           const int flip) {
+    for (int ks = 0; ks < kth; ++ks) {
+        const double a = lds_f64_dyn(pa);
+#pragma unroll
+        for (int q = 0; q < CNT; ++q) {
+            double b = lds_f64_dyn(pb + q * 128);
+            b = __hiloint2double(__double2hiint(b) ^ flip, __double2loint(b));
+            dmma_m8n8k4(acc[q][0], acc[q][1], a, b);
+        }
+        pa += 32;
+        pb += b_step;
+    }
+}
+template <int MAXT, int CNT>
+__device__ __forceinline__ void k1_t_dispatch(const int cnt, double (&acc)[MAXT][2], uint32_t pa, uint32_t pb, const int kth,
+                                              const uint32_t b_step, const int flip) {
+    if constexpr (CNT > 0) {
+        if (cnt == CNT) k1_t_kloop<MAXT, CNT>(acc, pa, pb, kth, b_step, flip);
+        else k1_t_dispatch<MAXT, CNT - 1>(cnt, acc, pa, pb, kth, b_step, flip);
+    }
 }
 
 // Build with -DAFQMC_K1_PHASE_CLOCKS to accumulate, over all CTAs of all launches, the clock64() time from CTA start to
@@ -329,23 +392,8 @@ __global__ void __launch_bounds__(K1_THREADS, BIG ? 1 : 4) k1_overlap_inverse_th
                 uint32_t pa = a_u + (g & 1) * L.psi_stage_bytes + s_st * 256 + lane * 8;
                 uint32_t pb = ring_u + (g & 1) * L.stage_bytes + fk * L.pitch + (8 * s_cb0 + fr) * 8;
                 const uint32_t im_off = 8u * L.ns * 256u;
-                for (int ks = 0; ks < nks; ++ks) {
-                    const double a = lds_f64_dyn(pa);
-                    const double a2 = cplx ? lds_f64_dyn(pa + im_off) : 0.0;
-#pragma unroll
-                    for (int q = 0; q < MAXT_S; ++q) {
-                        if (q < s_cnt) {
-                            const double b = lds_f64_dyn(pb + q * 64);
-                            dmma_m8n8k4(acc[q][0], acc[q][1], a, b);
-                            if (cplx) {    // + Im psi^T (phi_im, -phi_re): (a - ib)(x + iy) = (ax + by) + i(ay - bx)
-                                const double sw = lds_f64_dyn((pb + q * 64) ^ 8u);     // the other component of the same element
-                                dmma_m8n8k4(acc[q][0], acc[q][1], a2, (fr & 1) ? -sw : sw);
-                            }
-                        }
-                    }
-                    pa += L.ns * 256;
-                    pb += 4 * L.pitch;
-                }
+                if (cplx) k1_s_dispatch<MAXT_S, MAXT_S, true>(s_cnt, acc, pa, pb, nks, L.ns * 256, 4 * L.pitch, im_off, fr & 1);
+                else k1_s_dispatch<MAXT_S, MAXT_S, false>(s_cnt, acc, pa, pb, nks, L.ns * 256, 4 * L.pitch, im_off, fr & 1);
             }
         }
         __syncthreads();                                        // the ring and the psi fragments are free
@@ -367,7 +415,7 @@ __global__ void __launch_bounds__(K1_THREADS, BIG ? 1 : 4) k1_overlap_inverse_th
     K1_MARK(3);
 
     // ---- X = S^-1, result in W0 ------------------------------------------------------------------------------------------
-    const bool singular = !k1_gauss_jordan<BIG ? 16 : 4, BIG ? 6 : 5>(n, smem_u32((n & 1) ? W1 : W0), smem_u32((n & 1) ? W0 : W1),
+    const bool singular = !k1_gauss_jordan<BIG ? 16 : 4, BIG ? 6 : 5, K1_THREADS>(n, smem_u32((n & 1) ? W1 : W0), smem_u32((n & 1) ? W0 : W1),
                                                                       smem_u32(keys), rowof, pivs, tid);
     K1_MARK(4);
     // ---- the fragment-ordered inverse XF -------------------------------------------------------
@@ -434,19 +482,7 @@ __global__ void __launch_bounds__(K1_THREADS, BIG ? 1 : 4) k1_overlap_inverse_th
                 for (int q = 0; q < MAXT_T; ++q) { acc[q][0] = 0.0; acc[q][1] = 0.0; }
                 uint32_t pa = ring_u + (c & 1) * L.stage_bytes + (8 * t_s + fr) * L.pitch + fk * 8;
                 uint32_t pb = xf_u + cb0 * 128 + b_lane;
-                for (int ks = 0; ks < L.kth; ++ks) {
-                    const double a = lds_f64_dyn(pa);
-#pragma unroll
-                    for (int q = 0; q < MAXT_T; ++q) {
-                        if (q < cnt) {
-                            double b = lds_f64_dyn(pb + q * 128);
-                            b = __hiloint2double(__double2hiint(b) ^ flip, __double2loint(b));
-                            dmma_m8n8k4(acc[q][0], acc[q][1], a, b);
-                        }
-                    }
-                    pa += 32;
-                    pb += L.ncb * 128;
-                }
+                k1_t_dispatch<MAXT_T, MAXT_T>(cnt, acc, pa, pb, L.kth, L.ncb * 128, flip);
                 if (p < N) {
                     const long long prow = (long long)(p >> 2) * lay.strips * 32 + (p & 3);
 #pragma unroll

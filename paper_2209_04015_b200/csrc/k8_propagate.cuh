@@ -19,6 +19,7 @@
 //   k8_log_overlap         sum over spins of K1's log-determinants, arg wrapped to (-pi, pi]
 #pragma once
 #include <math_constants.h>
+#include <type_traits>
 #include "common.cuh"
 
 namespace afqmc {
@@ -268,38 +269,49 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
     const int nchunks = (N + K9_KC - 1) / K9_KC;
     load_chunk(0, 0);
     const int fr = lane >> 2, fk = lane & 3;
-    const double sgn = (fr & 1) ? 1.0 : -1.0;                                  // (i T)[q][c] = sgn * T[q][c ^ 1]
+    const int sgn_flip = (fr & 1) ? 0 : (int)0x80000000;                       // (i T)[q][c] = +- T[q][c ^ 1]: - on the even (re) columns
     for (int ch = 0; ch < nchunks; ++ch) {
         if (ch + 1 < nchunks) { load_chunk((ch + 1) & 1, (ch + 1) * K9_KC); cp_async_wait<1>(); }
         else cp_async_wait<0>();
         __syncthreads();
         const double *a = sA + (ch & 1) * (2 * K9_MAXROWS * K9_APITCH);
         const double *bb = sB + (ch & 1) * (K9_KC * K9_BPITCH);
-        if (my_mt > 0) {
+        // A predicated-off DMMA still occupies the tensor pipe, so the strip count (MM) and the complex second product are
+        // compile-time in the loop below and chosen by warp-uniform branches.
+        auto chunk_mma = [&](auto mm_tag, auto cx_tag) {
+            constexpr int MM = decltype(mm_tag)::value;
+            constexpr bool CX = decltype(cx_tag)::value;
 #pragma unroll
             for (int ks = 0; ks < K9_KC / 4; ++ks) {
-                double are[2], aim[2];
+                double are[MM], aim[MM];
 #pragma unroll
-                for (int m = 0; m < 2; ++m) {
+                for (int m = 0; m < MM; ++m) {
                     const int r = (warp + K9_WARPS * m) * 8 + fr;
-                    are[m] = (m < my_mt) ? a[r * K9_APITCH + ks * 4 + fk] : 0.0;
-                    aim[m] = (cplx && m < my_mt) ? a[(K9_MAXROWS + r) * K9_APITCH + ks * 4 + fk] : 0.0;
+                    are[m] = a[r * K9_APITCH + ks * 4 + fk];
+                    if constexpr (CX) aim[m] = a[(K9_MAXROWS + r) * K9_APITCH + ks * 4 + fk];
                 }
 #pragma unroll
                 for (int q = 0; q < K9_NT; ++q) {
-                    if (q < nt) {
-                        const double *bp = bb + (ks * 4 + fk) * K9_BPITCH + q * 8;
-                        const double b0 = bp[fr];
-                        dmma_m8n8k4(acc[0][q][0], acc[0][q][1], are[0], b0);
-                        if (my_mt > 1) dmma_m8n8k4(acc[1][q][0], acc[1][q][1], are[1], b0);
-                        if (cplx) {
-                            const double b1 = sgn * bp[fr ^ 1];
-                            dmma_m8n8k4(acc[0][q][0], acc[0][q][1], aim[0], b1);
-                            if (my_mt > 1) dmma_m8n8k4(acc[1][q][0], acc[1][q][1], aim[1], b1);
-                        }
+                    if (q >= nt) break;                                        // CTA-uniform early exit: a branch, never a predicate
+                    const double *bp = bb + (ks * 4 + fk) * K9_BPITCH + q * 8;
+                    const double b0 = bp[fr];
+#pragma unroll
+                    for (int m = 0; m < MM; ++m) dmma_m8n8k4(acc[m][q][0], acc[m][q][1], are[m], b0);
+                    if constexpr (CX) {
+                        const double t = bp[fr ^ 1];
+                        const double b1 = __hiloint2double(__double2hiint(t) ^ sgn_flip, __double2loint(t));
+#pragma unroll
+                        for (int m = 0; m < MM; ++m) dmma_m8n8k4(acc[m][q][0], acc[m][q][1], aim[m], b1);
                     }
                 }
             }
+        };
+        if (my_mt == 2) {
+            if (cplx) chunk_mma(std::integral_constant<int, 2>{}, std::true_type{});
+            else chunk_mma(std::integral_constant<int, 2>{}, std::false_type{});
+        } else if (my_mt == 1) {
+            if (cplx) chunk_mma(std::integral_constant<int, 1>{}, std::true_type{});
+            else chunk_mma(std::integral_constant<int, 1>{}, std::false_type{});
         }
         __syncthreads();
     }
