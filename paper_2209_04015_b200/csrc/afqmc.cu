@@ -848,10 +848,13 @@ int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *ch
     ctx->v_kps = (ksteps + ctx->v_ksc - 1) / ctx->v_ksc * ctx->v_ksc;
     ctx->v_nchunks = ctx->v_kps / ctx->v_ksc;
     ctx->v_nstages = 2;
-    const int rstrips = (2 * maxw + 7) / 8, rtiles = (rstrips + K2_MAX_WM - 1) / K2_MAX_WM;
-    ctx->v_strips = (rstrips + rtiles - 1) / rtiles;
-    const long long npq = (long long)N * (N + 1) / 2;             // upper triangle: L^g and A(y) are symmetric
-    ctx->v_n_ct = (int)((npq + 127) / 128);
+    // Rows of the GEMM are the pairs p <= q (upper triangle: L^g and A(y) are symmetric), 96 per tile, so that the big
+    // operand -- the Cholesky vectors, 8 Ngamma N (N + 1) / 2 bytes -- streams from HBM exactly once and every warp of
+    // the CTA owns a strip; columns are (walker, re / im) of the coefficients, 128 per tile.
+    const long long npq = (long long)N * (N + 1) / 2;
+    ctx->v_strips = K2_MAX_WM;
+    const int rtiles = (int)((npq + 8 * ctx->v_strips - 1) / (8 * ctx->v_strips));
+    ctx->v_n_ct = (2 * maxw + 127) / 128;
     ctx->ldv = (long long)ctx->v_n_ct * 128;
     ctx->v_smem = (size_t)ctx->v_nstages * ctx->v_ksc * (ctx->v_strips + 16) * 256 + (size_t)2 * ctx->v_nstages * 8 + 16;
     ctx->v_layA = OperandLayout{1, ctx->v_strips, ctx->v_kps, ctx->v_strips * 8, (long long)ctx->v_strips * ctx->v_kps * 32};
@@ -862,12 +865,12 @@ int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *ch
     CU_TRY(ctx, cudaMemsetAsync(ctx->v_A, 0, a_bytes, stream));
     CU_TRY(ctx, cudaMemsetAsync(ctx->v_B, 0, b_bytes, stream));
     if (ksteps > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_enable_propagation: n_gamma > 262140 is not supported");
-    k8_pack_chol_vhs<<<dim3((N + 127) / 128, N, ksteps), 128, 0, stream>>>(chol, N, n_gamma, ctx->v_layB, ctx->v_B);
+    k8_pack_chol_vhs<<<dim3((N + 127) / 128, N, ksteps), 128, 0, stream>>>(chol, N, n_gamma, ctx->v_layA, ctx->v_A);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 4 + 18 + nsq;
 
     // ---- work buffers ------------------------------------------------------------------------------------------------
-    CU_TRY(ctx, cudaMalloc(&ctx->Vtri, (size_t)2 * maxw * ctx->ldv * 8));
+    CU_TRY(ctx, cudaMalloc(&ctx->Vtri, (size_t)rtiles * 8 * ctx->v_strips * ctx->ldv * 8));      // [pair p <= q][(walker, re / im)]
     CU_TRY(ctx, cudaMalloc(&ctx->V, (size_t)2 * maxw * N * N * 8));
     CU_TRY(ctx, cudaMalloc(&ctx->fbuf, (size_t)maxw * n_gamma * 16));
     CU_TRY(ctx, cudaMalloc(&ctx->xbar, (size_t)maxw * n_gamma * 16));
@@ -906,22 +909,24 @@ int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *
 
     // (2) xbar (Eq. 9) and the coefficients of A(x - xbar); A(y)_w = sum_g c_wg L^g on the FP64 tensor cores
     const long long nf = (long long)n_walkers * ((n_gamma + 3) / 4);
-    k8_fields<<<(unsigned)((nf + 255) / 256), 256, 0, stream>>>(n_walkers, n_gamma, ctx->dt, ctx->fbuf, x, ctx->xbar, ctx->v_layA, ctx->v_A);
+    k8_fields<<<(unsigned)((nf + 255) / 256), 256, 0, stream>>>(n_walkers, n_gamma, ctx->dt, ctx->fbuf, x, ctx->xbar, ctx->v_layB, ctx->v_B);
     CU_TRY(ctx, cudaGetLastError());
     {
         K2FbParams p2{};
         p2.A = ctx->v_A; p2.B = ctx->v_B;
         p2.itemA_doubles = ctx->v_layA.tile_doubles; p2.tileB_doubles = ctx->v_layB.tile_doubles; p2.partB_doubles = 0;
-        p2.rows_per_tile = ctx->v_strips * 8; p2.rows_total = 2 * n_walkers;
+        const long long npq = (long long)N * (N + 1) / 2;
+        p2.rows_per_tile = ctx->v_strips * 8; p2.rows_total = (int)npq;
         p2.strips = ctx->v_strips; p2.WM = K2_MAX_WM;
         p2.kps = ctx->v_kps; p2.ksc = ctx->v_ksc; p2.nchunks = ctx->v_nchunks; p2.nstages = ctx->v_nstages;
-        p2.n_items_r = (2 * n_walkers + p2.rows_per_tile - 1) / p2.rows_per_tile; p2.ksplit = 1; p2.n_ct = ctx->v_n_ct;
+        p2.n_items_r = (int)((npq + p2.rows_per_tile - 1) / p2.rows_per_tile); p2.ksplit = 1; p2.n_ct = (2 * n_walkers + 127) / 128;
         p2.craw = ctx->Vtri;
         const long long ntiles = (long long)p2.n_items_r * p2.n_ct;
         k2_force_bias<16><<<(int)std::min<long long>(ntiles, ctx->num_sms), 32 * K2_MAX_WM, ctx->v_smem, stream>>>(p2);
         CU_TRY(ctx, cudaGetLastError());
-        if (2 * n_walkers > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_propagate: more than 32767 walkers per call");
-        k8_expand_symmetric<<<dim3((N + 127) / 128, N, 2 * n_walkers), 128, 0, stream>>>(ctx->Vtri, ctx->ldv, N, ctx->V);
+        if (N > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_propagate: N > 65535");
+        k8_expand_symmetric<<<dim3((N + 31) / 32, N, (2 * n_walkers + 31) / 32), dim3(32, 8), 0, stream>>>(
+            ctx->Vtri, (long long)p2.n_ct * 128, N, 2 * n_walkers, ctx->V);
         CU_TRY(ctx, cudaGetLastError());
     }
     CU_TRY(ctx, mark());

@@ -10,7 +10,7 @@
 //   k8_one_body_shift      h' = h - 1/2 sum_g L^g L^g                                  once per handle
 //   k8_pack_chol_vhs       chol [g][p<=q] -> B operand of the field GEMM (fragment order, upper triangle only) once per handle
 //   k8_fields              xbar, and the coefficients c_g = i sqrt(dt) (x_g - xbar_g) of A(y) as the GEMM's A operand
-//   (k2_force_bias<16>)    A(y)_w[p<=q] = sum_g c_wg L^g[pq]  -- a real GEMM [2 Nw x Ngamma].[Ngamma x N(N+1)/2] over the
+//   (k2_force_bias<16>)    A(y)_w[p<=q] = sum_g L^g[pq] c_wg  -- a real GEMM [N(N+1)/2 x Ngamma].[Ngamma x 2 Nw] over the
 //                          same TMA-fed operand ring as the force-bias GEMM (k2_exchange.cuh)
 //   k8_expand_symmetric    upper triangle -> full N x N planes for K9
 //   k9_apply               Out_w = alpha M_w In_w (+ running sum), M complex (planes) or real and shared: the Taylor terms
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(256) k8_one_body_shift(const double *__restric
 // for p <= q, N (N + 1) / 2 columns instead of N^2 -- half the flops and half the third packing of chol.
 __host__ __device__ inline long long tri_index(int p, int q, int N) { return (long long)p * N - (long long)p * (p - 1) / 2 + (q - p); }
 
-// chol [g][p][q], q >= p -> packed B operand: column t(p, q), tile = t / (8 strips), lane = (t % 8) * 4 + g % 4, k-step = g / 4.
+// chol [g][p][q], q >= p -> packed A operand of the field GEMM: row t(p, q), tile = t / (8 strips), lane = (t % 8) * 4 + g % 4, k-step = g / 4.
 // grid (ceil(N/128), N, ceil(Ngamma/4)): one thread per (p, q, group of 4 gamma); reads coalesced along q, 32-byte writes.
 __global__ void k8_pack_chol_vhs(const double *__restrict__ chol, int N, int n_gamma, OperandLayout lay,
                                  double *__restrict__ packed) {
@@ -68,17 +68,32 @@ __global__ void k8_pack_chol_vhs(const double *__restrict__ chol, int N, int n_g
     *reinterpret_cast<double2 *>(dst + 2) = make_double2(v[2], v[3]);
 }
 
-// Upper triangle [row][ldtri] -> full symmetric matrices [row][N][N]  (row = 2 w + plane).  grid (ceil(N/128), N, rows).
-__global__ void k8_expand_symmetric(const double *__restrict__ tri, long long ldtri, int N, double *__restrict__ full) {
-    const int q = blockIdx.x * blockDim.x + threadIdx.x, p = blockIdx.y;
-    if (q >= N) return;
-    const long long row = blockIdx.z;
-    const long long t = p <= q ? tri_index(p, q, N) : tri_index(q, p, N);
-    full[(row * N + p) * N + q] = tri[row * ldtri + t];
+// Field GEMM output [pair t(p, q), p <= q][ld] with column = 2 w + plane  ->  full symmetric matrices [2 w + plane][N][N].
+// grid (ceil(N/32), N, ceil(rows/32)), block (32, 8): a 32 (q) x 32 (matrix) tile goes through shared memory, so that both
+// the reads (32 consecutive columns of one pair) and the writes (32 consecutive q of one matrix row) are 256-byte segments.
+__global__ void __launch_bounds__(256) k8_expand_symmetric(const double *__restrict__ tri, long long ld, int N, int rows,
+                                                           double *__restrict__ full) {
+    __shared__ double tile[32][33];
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int q0 = blockIdx.x * 32, p = blockIdx.y, row0 = blockIdx.z * 32;
+    for (int jj = ty; jj < 32; jj += 8) {
+        const int q = q0 + jj;
+        double v = 0.0;
+        if (q < N && row0 + tx < rows) {
+            const long long t = p <= q ? tri_index(p, q, N) : tri_index(q, p, N);
+            v = tri[t * ld + row0 + tx];
+        }
+        tile[jj][tx] = v;
+    }
+    __syncthreads();
+    for (int ii = ty; ii < 32; ii += 8) {
+        const int row = row0 + ii, q = q0 + tx;
+        if (row < rows && q < N) full[((long long)row * N + p) * N + q] = tile[tx][ii];
+    }
 }
 
 // xbar_wg = -i sqrt(dt) fb_wg (Eq. 9);  c_wg = i sqrt(dt) (x_wg - xbar_wg) = -dt fb_wg + i sqrt(dt) x_wg.
-// Writes xbar [Nw][Ngamma] complex and the GEMM's A operand: row 2w = Re c_w, row 2w + 1 = Im c_w, k = gamma.
+// Writes xbar [Nw][Ngamma] complex and the field GEMM's B operand: column 2w = Re c_w, column 2w + 1 = Im c_w, k = gamma.
 __global__ void k8_fields(int n_walkers, int n_gamma, double dt, const double *__restrict__ fb /* [Nw][Ng][2] */,
                           const double *__restrict__ x /* [Nw][Ng] */, double *__restrict__ xbar, OperandLayout lay,
                           double *__restrict__ packedA) {
