@@ -374,11 +374,11 @@ int launch_force_bias_gemm(afqmc_ctx *ctx, int n_walkers, double *out, cudaStrea
     return AFQMC_OK;
 }
 
-// One K9 launch: Out_b = alpha M_b In_b (+ Sum_b), b = 0 .. batch-1.
+// One K9 launch: Out_b = alpha M_b In_b, b = 0 .. batch-1; optionally Sum_b += Out_b, or Out_b = Add_b + alpha M_b In_b.
 int launch_k9(afqmc_ctx *ctx, const double *Mre, const double *Mim, long long m_stride, int ldm, const double *In, double *Out,
-              double *Sum, long long io_stride, int ld, int C, int batch, double alpha, cudaStream_t stream) {
+              double *Sum, long long io_stride, int ld, int C, int batch, double alpha, cudaStream_t stream, const double *Add = nullptr) {
     K9Params p{};
-    p.Mre = Mre; p.Mim = Mim; p.m_batch_stride = m_stride; p.ldm = ldm; p.In = In; p.Out = Out; p.Sum = Sum;
+    p.Mre = Mre; p.Mim = Mim; p.m_batch_stride = m_stride; p.ldm = ldm; p.In = In; p.Out = Out; p.Sum = Sum; p.Add = Add;
     p.io_batch_stride = io_stride; p.ld = ld; p.N = ctx->N; p.C = C; p.rt_strips = ctx->p_rt_strips; p.alpha = alpha;
     // column groups: as few as fit the accumulators, of equal width (splitting further to fill the last wave of CTAs was
     // measured and lost: 5.6 vs 4.7 ms for the Taylor phase at cu2o2, the M tile is then staged twice)
@@ -798,7 +798,7 @@ int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *ch
     ctx->dt = dt;
     ctx->ldE = (N + 1) & ~1; ctx->ldt = C;                        // even pitches: K9 stores (re, im) pairs as double2
     const int S = (N + 7) / 8;
-    ctx->p_row_tiles = (S + 2 * K9_WARPS - 1) / (2 * K9_WARPS);
+    ctx->p_row_tiles = (S + K9_MAXROWS / 8 - 1) / (K9_MAXROWS / 8);
     ctx->p_rt_strips = (S + ctx->p_row_tiles - 1) / ctx->p_row_tiles;
     CU_TRY(ctx, allow_max_smem(k9_apply));
     CU_TRY(ctx, allow_max_smem(k2_force_bias<16>));
@@ -936,14 +936,18 @@ int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *
     const long long np = (long long)n_walkers * N * ld;
     k8_pack_walkers<<<(unsigned)((np + 255) / 256), 256, 0, stream>>>(reinterpret_cast<const double *>(walkers), n_walkers, N, na, nb, ld, X0);
     CU_TRY(ctx, cudaGetLastError());
-    if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, X0, X1, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;
-    CU_TRY(ctx, cudaMemcpyAsync(X0, X1, (size_t)np * 8, cudaMemcpyDeviceToDevice, stream));          // running sum S = T0
-    double *cur = X1, *nxt = X2;
-    for (int k = 1; k <= taylor_order; ++k) {
-        if (int rc = launch_k9(ctx, ctx->V, ctx->V + (long long)N * N, 2LL * N * N, N, cur, nxt, X0, tstride, ld, C, n_walkers, 1.0 / k, stream)) return rc;
-        std::swap(cur, nxt);
+    if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, X0, X1, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;   // T0 = E phi
+    // sum_{k <= order} A^k T0 / k!  by Horner's rule:  R_order = T0,  R_{j-1} = T0 + A R_j / j,  result R_0  (the same
+    // polynomial as the term-by-term sum; one read of T0 per step instead of a read-modify-write of a running sum)
+    const double *R = X1;
+    double *bufs[2] = {X0, X2};
+    for (int j = taylor_order; j >= 1; --j) {
+        double *out = bufs[(taylor_order - j) & 1];
+        if (int rc = launch_k9(ctx, ctx->V, ctx->V + (long long)N * N, 2LL * N * N, N, R, out, nullptr, tstride, ld, C, n_walkers, 1.0 / j, stream, X1)) return rc;
+        R = out;
     }
-    if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, X0, cur, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;
+    double *cur = (R == X0) ? X2 : X0;                            // any buffer other than R (X1 is free after the last step too)
+    if (int rc = launch_k9(ctx, ctx->Emat, nullptr, 0, ctx->ldE, R, cur, nullptr, tstride, ld, C, n_walkers, 1.0, stream)) return rc;
     const long long nu = (long long)n_walkers * N * C;
     k8_unpack_walkers<<<(unsigned)((nu + 255) / 256), 256, 0, stream>>>(cur, n_walkers, N, na, nb, ld, reinterpret_cast<double *>(walkers));
     CU_TRY(ctx, cudaGetLastError());

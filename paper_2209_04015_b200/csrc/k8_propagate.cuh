@@ -188,17 +188,20 @@ __global__ void k8_set_diagonal(double *M, int N, int ld, double s) {
 constexpr int K9_THREADS = 384;
 constexpr int K9_WARPS = K9_THREADS / 32;
 constexpr int K9_KC = 16;             // q per chunk = 4 DMMA k-steps
-constexpr int K9_MAXROWS = 192;       // 24 strips
+constexpr int K9_MAXROWS = 160;       // 20 strips: warps 0-7 own two, warps 8-11 one (K2's shape)
 constexpr int K9_NT = 13;             // column blocks per group
 constexpr int K9_APITCH = 20, K9_BPITCH = 116;
-constexpr int K9_SMEM = 2 * (2 * K9_MAXROWS * K9_APITCH + K9_KC * K9_BPITCH) * 8;
+constexpr int K9_STAGES = 3;
+constexpr int K9_STAGE_DOUBLES = 2 * K9_MAXROWS * K9_APITCH + K9_KC * K9_BPITCH;
+constexpr int K9_SMEM = K9_STAGES * K9_STAGE_DOUBLES * 8;
 
 struct K9Params {
     const double *Mre, *Mim;
     long long m_batch_stride;
     int ldm;
     const double *In;
-    double *Out, *Sum;               // Sum may be nullptr
+    double *Out, *Sum;               // Sum may be nullptr: Sum += Out (running sum of a series)
+    const double *Add;               // may be nullptr: Out = Add + alpha M In (a Horner step); not together with Sum
     long long io_batch_stride;
     int ld;                          // even
     int N, C;                        // M is N x N; In has C real columns in use
@@ -218,8 +221,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads x 168 registers = the register file
     extern __shared__ __align__(16) unsigned char k9_smem[];
-    double *sA = reinterpret_cast<double *>(k9_smem);                          // [2 stages][2 planes][192][20]
-    double *sB = sA + 2 * 2 * K9_MAXROWS * K9_APITCH;                          // [2 stages][16][116]
+    double *sS = reinterpret_cast<double *>(k9_smem);                          // [3 stages]{ A [2 planes][160][20], B [16][116] }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int N = P.N, b = blockIdx.z;
     const int row0 = blockIdx.x * P.rt_strips * 8;
@@ -250,8 +252,8 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
     }
 
     auto load_chunk = [&](int stage, int q0) {
-        double *a = sA + stage * (2 * K9_MAXROWS * K9_APITCH);
-        double *bb = sB + stage * (K9_KC * K9_BPITCH);
+        double *a = sS + stage * K9_STAGE_DOUBLES;
+        double *bb = a + 2 * K9_MAXROWS * K9_APITCH;
         const int qa = q0 + a_piece;
         for (int pl = 0; pl < nplanes; ++pl) {
             const double *M = pl ? Mim : Mre;
@@ -281,16 +283,21 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
 #pragma unroll
         for (int q = 0; q < K9_NT; ++q) { acc[m][q][0] = 0.0; acc[m][q][1] = 0.0; }
 
+    // Three stages, one CTA barrier per chunk: the barrier at the top of chunk ch says "chunk ch has landed and everybody
+    // is done with chunk ch - 1", after which every warp computes chunk ch and THEN issues the copies of chunk ch + 2 into
+    // the stage chunk ch - 1 occupied -- so the warps issue their copies at different times and the tensor pipe never
+    // waits for all twelve of them to get through the address arithmetic.
     const int nchunks = (N + K9_KC - 1) / K9_KC;
     load_chunk(0, 0);
+    if (nchunks > 1) load_chunk(1, K9_KC);
     const int fr = lane >> 2, fk = lane & 3;
     const int sgn_flip = (fr & 1) ? 0 : (int)0x80000000;                       // (i T)[q][c] = +- T[q][c ^ 1]: - on the even (re) columns
     for (int ch = 0; ch < nchunks; ++ch) {
-        if (ch + 1 < nchunks) { load_chunk((ch + 1) & 1, (ch + 1) * K9_KC); cp_async_wait<1>(); }
+        if (ch + 1 < nchunks) cp_async_wait<1>();
         else cp_async_wait<0>();
         __syncthreads();
-        const double *a = sA + (ch & 1) * (2 * K9_MAXROWS * K9_APITCH);
-        const double *bb = sB + (ch & 1) * (K9_KC * K9_BPITCH);
+        const double *a = sS + (ch % K9_STAGES) * K9_STAGE_DOUBLES;
+        const double *bb = a + 2 * K9_MAXROWS * K9_APITCH;
         // A predicated-off DMMA still occupies the tensor pipe, so the strip count (MM) and the complex second product are
         // compile-time in the loop below and chosen by warp-uniform branches.
         auto chunk_mma = [&](auto mm_tag, auto cx_tag) {
@@ -305,15 +312,20 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
                     are[m] = a[r * K9_APITCH + ks * 4 + fk];
                     if constexpr (CX) aim[m] = a[(K9_MAXROWS + r) * K9_APITCH + ks * 4 + fk];
                 }
+                // Re(M) pass over all column blocks, then Im(M) pass: two DMMAs on one accumulator are then a whole pass
+                // (13 MM instructions) apart, never back to back.
 #pragma unroll
                 for (int q = 0; q < K9_NT; ++q) {
                     if (q >= nt) break;                                        // CTA-uniform early exit: a branch, never a predicate
-                    const double *bp = bb + (ks * 4 + fk) * K9_BPITCH + q * 8;
-                    const double b0 = bp[fr];
+                    const double b0 = bb[(ks * 4 + fk) * K9_BPITCH + q * 8 + fr];
 #pragma unroll
                     for (int m = 0; m < MM; ++m) dmma_m8n8k4(acc[m][q][0], acc[m][q][1], are[m], b0);
-                    if constexpr (CX) {
-                        const double t = bp[fr ^ 1];
+                }
+                if constexpr (CX) {
+#pragma unroll
+                    for (int q = 0; q < K9_NT; ++q) {
+                        if (q >= nt) break;
+                        const double t = bb[(ks * 4 + fk) * K9_BPITCH + q * 8 + (fr ^ 1)];
                         const double b1 = __hiloint2double(__double2hiint(t) ^ sgn_flip, __double2loint(t));
 #pragma unroll
                         for (int m = 0; m < MM; ++m) dmma_m8n8k4(acc[m][q][0], acc[m][q][1], aim[m], b1);
@@ -328,11 +340,12 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
             if (cplx) chunk_mma(std::integral_constant<int, 1>{}, std::true_type{});
             else chunk_mma(std::integral_constant<int, 1>{}, std::false_type{});
         }
-        __syncthreads();
+        if (ch + 2 < nchunks) load_chunk((ch + 2) % K9_STAGES, (ch + 2) * K9_KC);
     }
 
     double *Out = P.Out + (long long)b * P.io_batch_stride;
     double *Sum = P.Sum ? P.Sum + (long long)b * P.io_batch_stride : nullptr;
+    const double *Add = P.Add ? P.Add + (long long)b * P.io_batch_stride : nullptr;
 #pragma unroll
     for (int m = 0; m < 2; ++m) {
         if (m >= my_mt) continue;
@@ -343,7 +356,11 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
             const int c = q * 8 + 2 * fk;
             if (q < nt && c < ncols) {                                          // ld is even and C is even or padded: (c, c+1) stay inside the row
                 const long long off = (long long)(row0 + r) * P.ld + col0 + c;
-                const double2 v = make_double2(P.alpha * acc[m][q][0], P.alpha * acc[m][q][1]);
+                double2 v = make_double2(P.alpha * acc[m][q][0], P.alpha * acc[m][q][1]);
+                if (Add) {
+                    const double2 t0 = *reinterpret_cast<const double2 *>(Add + off);
+                    v.x += t0.x; v.y += t0.y;
+                }
                 *reinterpret_cast<double2 *>(Out + off) = v;
                 if (Sum) {
                     double2 s = *reinterpret_cast<double2 *>(Sum + off);
