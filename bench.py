@@ -314,11 +314,11 @@ def main():
         le.set_profiling(False)
         ms_prop = max_over_ranks(e0.elapsed_time(e1)) / args.steps
         ne = inp.n_alpha + inp.n_beta
-        flops_field = 4.0 * nw * inp.n_gamma * inp.N * (inp.N + 1) / 2         # [2Nw x Ng].[Ng x N(N+1)/2] real GEMM (L symmetric)
+        flops_field = 4.0 * nw * inp.n_gamma * inp.N * (inp.N + 1) / 2         # [N(N+1)/2 x Ng].[Ng x 2Nw] real GEMM (L symmetric)
         flops_taylor = (PROP_ORDER * 8.0 + 2 * 4.0) * inp.N ** 2 * ne * nw      # complex A T_k terms + two real E T products
         prop = {"value": world * nw / (ms_prop * 1e-3), "unit": UNIT, "ms_per_step": ms_prop, "dt": PROP_DT,
                 "taylor_order": PROP_ORDER,
-                "what": "afqmc_propagate: K1 + force-bias GEMM + field GEMM [2Nw x Ng].[Ng x N(N+1)/2] + (order + 2) batched "
+                "what": "afqmc_propagate: K1 + force-bias GEMM + field GEMM [N(N+1)/2 x Ng].[Ng x 2Nw] + (order + 2) batched "
                         "[N x N].[N x 2(na+nb)] products + K1 + phaseless weights; device-resident, x drawn beforehand",
                 "phase_ms": {"k1_overlap": phase[0], "force_bias_gemm": phase[1], "fields_and_field_gemm": phase[2],
                              "one_body_and_taylor": phase[3], "k1_and_weights": phase[4]},
@@ -373,7 +373,8 @@ def main():
                 "k1": {"algorithmic_bytes": int(walkers_bytes + info["theta_bytes"]),
                        "achieved_gbs": (walkers_bytes + info["theta_bytes"]) / (kms[0] * 1e-3) * 1e-9,
                        "hbm_peak_gbs": hbm_gbs,
-                       "note": "1 % of the step; bound by the latency of the shared-memory LU, not by HBM"}}
+                       "note": "0.5 % of the step; its two products run on the tensor pipe, the inversion between them is "
+                               "bound by dependent-issue latency (DESIGN.md section 6), not by HBM"}}
 
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N=1 only) ---------------------------------------
     cpu = None

@@ -189,8 +189,8 @@ int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const v
  *                 truncation error, about ||A||^(order+1) / (order+1)!, is the caller's to bound; the paper does not
  *                 state an order (6 is customary for dt ~ 0.005 and molecular Hamiltonians).
  *   Kernels, all on `stream`, no host synchronisation: K1 (theta, overlap of phi), force-bias GEMM, field GEMM
- *   [2 n_walkers x n_gamma].[n_gamma x N(N+1)/2] on the FP64 tensor cores, order + 2 batched [N x N].[N x 2(n_alpha+n_beta)]
- *   products, K1 again (overlap of phi'), weight update.  A walker orthogonal to the trial before or after the step gets
+ *   [N(N+1)/2 x n_gamma].[n_gamma x 2 n_walkers] on the FP64 tensor cores, order + 2 batched [N x N].[N x 2(n_alpha+n_beta)]
+ *   products (the series by Horner's rule), K1 again (overlap of phi'), weight update.  A walker orthogonal to the trial before or after the step gets
  *   weight NaN (its log-overlap is -inf).  Afterwards the handle's theta belongs to phi' (afqmc_spin_squared,
  *   afqmc_greens_function refer to the propagated walkers; afqmc_force_bias has nothing to return).
  *
