@@ -37,7 +37,6 @@ struct SpinCfg {
     int MT = 0, NT = 0, WM = 0, gT = 0, wT = 0, strips = 0, ksc = 0, nchunks = 0, nstages = 0, H = 0, LD2 = 0;
     int n_rt = 0, n_ct_max = 0;
     int ctas_per_sm = 1;                          // persistent K2 CTAs per SM (2: two half-size CTAs, epilogues overlap K loops)
-    bool uniform = false;                         // 20-strip tile: every warp one strip + a share of the other eight (k2_exchange_u)
     size_t k2_smem = 0, k1_smem = 0;
     OperandLayout layA{}, layB{};
     double *A = nullptr, *B = nullptr, *psi = nullptr, *ht = nullptr, *tbuf = nullptr, *xpart = nullptr;
@@ -213,10 +212,6 @@ bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
         }
     }
     if (best < 0) return false;
-    {
-        const char *u = std::getenv("AFQMC_K2_UNIFORM");
-        c.uniform = u && u[0] == '1' && c.strips == 20 && c.WM == K2_MAX_WM && c.MT == 2 && c.NT >= 5 && c.NT <= 13;
-    }
     c.nchunks = (ksteps + c.ksc - 1) / c.ksc;
     c.n_rt = (n_gamma + c.gT - 1) / c.gT;
     c.n_ct_max = (maxw + c.wT - 1) / c.wT;
@@ -253,18 +248,6 @@ K2Fn k2_pick(int mt, int nt) {
     }
     return nullptr;
 }
-
-// Uniform-work variant (k2_exchange_u): 20-strip tiles only.
-template <int NT>
-K2Fn k2_pick_u_nt(int nt) {
-    if constexpr (NT < 5) {
-        return nullptr;
-    } else {
-        if (nt == NT) return k2_exchange_u<NT>;
-        return k2_pick_u_nt<NT - 1>(nt);
-    }
-}
-K2Fn k2_pick_u(int nt) { return k2_pick_u_nt<13>(nt); }
 
 using K2FbFn = void (*)(const K2FbParams);
 template <int NT>
@@ -516,7 +499,7 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
             CR_TRY(cudaGetLastError());
             c->launches += 2;
         }
-        K2Fn fn = sc.uniform ? k2_pick_u(sc.NT) : k2_pick(sc.MT, sc.NT);
+        K2Fn fn = k2_pick(sc.MT, sc.NT);
         if (!fn) {
             free_ctx(c);
             return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_create: no K2 instantiation for MT=%d NT=%d", sc.MT, sc.NT);
@@ -559,7 +542,7 @@ static int launch_k2(afqmc_ctx *ctx, int s, int w0, int count, cudaStream_t stre
     p2.tbuf = sc.tbuf + (long long)w0 * ctx->n_gamma * 2; p2.xpart = sc.xpart + (long long)w0 * 2;
     const long long ntiles = (long long)p2.n_rt * p2.n_ct;
     const int grid = (int)std::min<long long>(ntiles, (long long)ctx->num_sms * sc.ctas_per_sm);
-    K2Fn fn = sc.uniform ? k2_pick_u(sc.NT) : k2_pick(sc.MT, sc.NT);
+    K2Fn fn = k2_pick(sc.MT, sc.NT);
     fn<<<grid, 32 * sc.WM, sc.k2_smem, stream>>>(p2);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;

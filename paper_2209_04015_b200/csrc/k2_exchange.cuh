@@ -367,287 +367,6 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Uniform variant for 20-strip tiles (the Cu2O2-scale shape): with strips dealt whole, eight warps carry two strips and four
-// carry one, so a ring lets the one-strip warps run ahead and stall, and the tensor pipe is fed by two warps per
-// sub-partition for part of the time (profiles/r2_k2_ablations.md).  Here every warp owns ONE whole strip (strip = warp)
-// and the eight remaining strips are shared by column blocks: sub-partition s (warps s, s + 4, s + 8) takes strips
-// X = 12 + 2 s and Y = 13 + 2 s, whose 2 NT tiles go to its three warps as C0 + (X1 + Y1) + C2, equal to within one tile.
-template <int NT>
-struct K2Uniform {
-    static constexpr int C0 = (2 * NT + 2) / 3;            // role 0: blocks [0, C0) of X
-    static constexpr int X1 = NT - C0;                     // role 1: blocks [C0, NT) of X ...
-    static constexpr int C1 = (2 * NT - C0 + 1) / 2;
-    static constexpr int Y1 = C1 - X1;                     //         ... and blocks [0, Y1) of Y
-    static constexpr int C2 = NT - Y1;                     // role 2: blocks [Y1, NT) of Y
-    static_assert(C0 <= NT && X1 >= 0 && Y1 >= 0 && Y1 <= NT && C1 <= C0 && C2 <= C0, "K2Uniform: bad split");
-};
-
-template <int ROLE, int NT, class Produce>
-__device__ __forceinline__ void k2_tile_mma_u(double (&accA)[NT][2], double (&accE)[K2Uniform<NT>::C0][2], K2Ring &R, const uint32_t frag_own,
-                                              const uint32_t frag_x, const uint32_t frag_y, const bool producer_warp, Produce &produce_poll,
-                                              const int lane) {
-    using U = K2Uniform<NT>;
-#pragma unroll 1
-    for (int c = 0; c < R.nchunks; ++c) {
-        const int nks = (c == R.nchunks - 1) ? R.last_ks : R.ksc;
-        if (producer_warp) {
-            if (lane == 0) produce_poll();
-            __syncwarp();
-        }
-        k2_wait_full(R.full_bar + 8u * R.stage, R.phase, producer_warp, lane, produce_poll);
-        const uint32_t base = R.smem_base + R.stage * R.stage_bytes;
-        uint32_t pa = base + frag_own, px = base + frag_x, py = base + frag_y;
-        uint32_t pb = base + R.a_chunk_bytes + 8u * lane;
-#pragma unroll 1
-        for (int ks = 0; ks < nks; ++ks) {
-            double b[NT];
-            const double a0 = lds_f64<0>(pa);
-            double ax = 0.0, ay = 0.0;
-            if constexpr (ROLE <= 1) ax = lds_f64<0>(px);
-            if constexpr (ROLE >= 1) ay = lds_f64<0>(py);
-#pragma unroll
-            for (int q = 0; q < NT; ++q) b[q] = lds_f64<0>(pb + q * 256);
-#pragma unroll
-            for (int q = 0; q < NT; ++q) dmma_m8n8k4(accA[q][0], accA[q][1], a0, b[q]);
-            if constexpr (ROLE == 0) {
-#pragma unroll
-                for (int q = 0; q < U::C0; ++q) dmma_m8n8k4(accE[q][0], accE[q][1], ax, b[q]);
-            } else if constexpr (ROLE == 1) {
-#pragma unroll
-                for (int q = 0; q < U::X1; ++q) dmma_m8n8k4(accE[q][0], accE[q][1], ax, b[U::C0 + q]);
-#pragma unroll
-                for (int q = 0; q < U::Y1; ++q) dmma_m8n8k4(accE[U::X1 + q][0], accE[U::X1 + q][1], ay, b[q]);
-            } else {
-#pragma unroll
-                for (int q = 0; q < U::C2; ++q) dmma_m8n8k4(accE[q][0], accE[q][1], ay, b[U::Y1 + q]);
-            }
-            pa += R.a_kstride; px += R.a_kstride; py += R.a_kstride;
-            pb += NT * 256u;
-        }
-        __syncwarp();
-        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(R.empty_bar + 8u * R.stage) : "memory");
-        if (++R.stage == R.nstages) { R.stage = 0; R.phase ^= 1u; }
-    }
-}
-
-template <int NT>
-__global__ void __maxnreg__(168) k2_exchange_u(const K2Params P) {   // blockDim = 384, strips = 20
-    extern __shared__ __align__(128) unsigned char k2_smem[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int WM = P.WM, n = P.n, H = P.H, LD2 = P.LD2;
-
-    const uint32_t a_chunk_bytes = (uint32_t)P.ksc * P.strips * 256u;
-    const uint32_t b_chunk_bytes = (uint32_t)P.ksc * NT * 256u;
-    const uint32_t stage_bytes = a_chunk_bytes + b_chunk_bytes;
-    unsigned char *stage_base = k2_smem;
-    double *staging = reinterpret_cast<double *>(k2_smem + (size_t)P.nstages * stage_bytes);   // [4*strips][LD2]
-    double *red = staging + (size_t)P.strips * 4 * LD2;                                         // [2][K2_MAX_WT][K2_MAX_WM][2]
-    uint64_t *full_bar = reinterpret_cast<uint64_t *>(red + 2 * K2_MAX_WT * K2_MAX_WM * 2);
-    uint64_t *empty_bar = full_bar + P.nstages;
-    uint64_t *stg_full = empty_bar + P.nstages;          // every warp has parked its accumulators of this tile
-    uint64_t *stg_free = stg_full + 1;                   // every warp is done reading the staging buffer
-    const int mma_warps = min(WM, P.strips);             // warps that own at least one strip
-    if (tid == 0) {
-        for (int s = 0; s < P.nstages; ++s) {
-            mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], mma_warps);
-        }
-        mbar_init(stg_full, WM);
-        mbar_init(stg_free, WM);
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    const int last_ks = P.ksteps - (P.nchunks - 1) * P.ksc;
-    // Tiles are dealt round-robin, tile index t = rt * n_ct + ct; a CTA steps from t to t + gridDim.x with two adds
-    // and a compare (no division on the per-chunk path).
-    const int step_rt = (int)(gridDim.x / (unsigned)P.n_ct), step_ct = (int)(gridDim.x % (unsigned)P.n_ct);
-    const int first_rt = (int)(blockIdx.x / (unsigned)P.n_ct), first_ct = (int)(blockIdx.x % (unsigned)P.n_ct);
-
-    // ---- producer: lane 0 of the last strip-owning warp (an epilogue warp, so it has slack).  It issues 1-D bulk async copies (TMA engine) of whole K-chunks of the packed
-    // operands into the ring.  It never blocks: once per k-step (and while it waits for its own data) it tests the
-    // empty barrier of the next stage to refill and issues the copies if every strip-owning warp has released it.
-    const bool producer_warp = (warp == mma_warps - 1);
-    int p_rt = first_rt, p_ct = first_ct, p_chunk = 0, p_stage = 0;
-    uint32_t p_phase = 0;
-    const double *p_a = P.A + (long long)p_rt * P.tileA_doubles;
-    const double *p_b = P.B + (long long)p_ct * P.tileB_doubles;
-    auto produce_poll = [&]() {
-        if (p_rt >= P.n_rt) return;
-        if (!mbar_test_addr(smem_u32(&empty_bar[p_stage]), p_phase ^ 1u)) return;
-        const bool last = (p_chunk == P.nchunks - 1);
-        const uint32_t ab = last ? (uint32_t)last_ks * P.strips * 256u : a_chunk_bytes;
-        const uint32_t bb = last ? (uint32_t)last_ks * NT * 256u : b_chunk_bytes;
-        mbar_arrive_expect_tx(&full_bar[p_stage], ab + bb);
-        unsigned char *dst = stage_base + (size_t)p_stage * stage_bytes;
-        bulk_g2s(dst, p_a, ab, &full_bar[p_stage]);
-        bulk_g2s(dst + a_chunk_bytes, p_b, bb, &full_bar[p_stage]);
-        p_a += a_chunk_bytes / 8; p_b += b_chunk_bytes / 8;
-        if (++p_stage == P.nstages) { p_stage = 0; p_phase ^= 1u; }
-        if (last) {
-            p_chunk = 0;
-            p_rt += step_rt; p_ct += step_ct;
-            if (p_ct >= P.n_ct) { p_ct -= P.n_ct; ++p_rt; }
-            p_a = P.A + (long long)p_rt * P.tileA_doubles;
-            p_b = P.B + (long long)p_ct * P.tileB_doubles;
-        } else {
-            ++p_chunk;
-        }
-    };
-    if (producer_warp && lane == 0)
-        for (int d = 0; d < P.nstages; ++d) produce_poll();     // fresh barriers: fills the whole ring
-
-    // ---- every warp: its own strip `warp` (all NT column blocks) plus an equal share of the eight extra strips --------
-    const int sub = warp & 3, role = warp >> 2;                  // SM sub-partition, role within it
-    const int stripX = 12 + 2 * sub, stripY = 13 + 2 * sub;
-
-    K2Ring R;
-    R.smem_base = smem_u32(stage_base); R.stage_bytes = stage_bytes; R.a_chunk_bytes = a_chunk_bytes;
-    asm volatile("" : "+r"(R.smem_base));      // opaque: keeps the window address in a register (no S2R per chunk)
-    R.a_kstride = (uint32_t)P.strips * 256u;
-    R.full_bar = smem_u32(full_bar); R.empty_bar = smem_u32(empty_bar);
-    asm volatile("" : "+r"(R.full_bar), "+r"(R.empty_bar));
-    R.nstages = P.nstages; R.ksc = P.ksc; R.nchunks = P.nchunks; R.last_ks = last_ks; R.ksteps = P.ksteps;
-    R.stage = 0; R.phase = 0;
-    const uint32_t frag_own = (uint32_t)warp * 256u + 8u * lane;
-    const uint32_t frag_x = (uint32_t)stripX * 256u + 8u * lane, frag_y = (uint32_t)stripY * 256u + 8u * lane;
-
-    // The tile loop is instantiated per role so that the K loop carries no predication.
-    auto run_tiles = [&](auto role_tag) {
-        constexpr int ROLE = decltype(role_tag)::value;
-        using U = K2Uniform<NT>;
-        uint32_t tpar = 0;                                      // parity of this CTA's tile counter
-        for (int rt = first_rt, ct = first_ct; rt < P.n_rt;) {
-            double accA[NT][2], accE[U::C0][2];
-#pragma unroll
-            for (int q = 0; q < NT; ++q) { accA[q][0] = 0.0; accA[q][1] = 0.0; }
-#pragma unroll
-            for (int q = 0; q < U::C0; ++q) { accE[q][0] = 0.0; accE[q][1] = 0.0; }
-            k2_tile_mma_u<ROLE, NT>(accA, accE, R, frag_own, frag_x, frag_y, producer_warp, produce_poll, lane);
-
-            // ------------------------------ epilogue ------------------------------
-            // Phase 1 (all warps): park the accumulators in the whole-tile staging buffer with the tile's own
-            // row/column numbering (row = g*nb + i, col = (plane*wT + wl)*n + j).  Rows are stored in pairs:
-            //     element (row, col)  ->  (row >> 1) * LD2 + (row & 1) * H + col,     H = 8 mod 16,  LD2 = 1 mod 16,
-            // which makes the fragment-order stores here, the row loads and the column loads of phase 2 all
-            // bank-conflict free (column loads 2-way when g*n is odd).
-            mbar_wait(stg_free, tpar ^ 1u);                                    // previous tile has been read out
-            {
-                auto park = [&](int strip, int q, const double (&v)[2]) {
-                    const int row = strip * 8 + (lane >> 2);
-                    double *dst = staging + (row >> 1) * LD2 + (row & 1) * H + 2 * (lane & 3) + q * 8;
-                    dst[0] = v[0]; dst[1] = v[1];
-                };
-#pragma unroll
-                for (int q = 0; q < NT; ++q) park(warp, q, accA[q]);
-                if constexpr (ROLE == 0) {
-#pragma unroll
-                    for (int q = 0; q < U::C0; ++q) park(stripX, q, accE[q]);
-                } else if constexpr (ROLE == 1) {
-#pragma unroll
-                    for (int q = 0; q < U::X1; ++q) park(stripX, U::C0 + q, accE[q]);
-#pragma unroll
-                    for (int q = 0; q < U::Y1; ++q) park(stripY, q, accE[U::X1 + q]);
-                } else {
-#pragma unroll
-                    for (int q = 0; q < U::C2; ++q) park(stripY, U::Y1 + q, accE[q]);
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(stg_full);
-            {
-                // Phase 2 (all warps, once the whole tile is parked; the FP64 pipe is shared with the DMMAs, so these
-                // DFMAs are only cheap while no warp is feeding it DMMAs): one (gamma g, walker wl) block
-                // T = R + iI (n x n) per pass, lanes over j, loop over i:
-                //     Re x += R_ij R_ji - I_ij I_ji,    Im x += 2 R_ij I_ji   (sum_ij I_ij R_ji = sum_ij R_ij I_ji by relabelling),
-                //     t = sum_j T_jj.
-                // When the tile has fewer blocks than warps, each block's i range is split into `rs` parts.
-                const int g0 = rt * P.gT;
-                const int gvalid = min(P.gT, P.n_gamma - g0);
-                const int w0 = ct * P.wT;
-                const int wvalid = min(P.wT, P.n_walkers - w0);
-                const int planeoff = P.wT * n;
-                const int nblk = gvalid * wvalid;
-                const int rs = max(1, WM / nblk);
-                double *redp = red + tpar * (K2_MAX_WT * K2_MAX_WM * 2);      // double-buffered by tile parity
-                if (lane < K2_MAX_WT) { redp[(lane * K2_MAX_WM + warp) * 2] = 0.0; redp[(lane * K2_MAX_WM + warp) * 2 + 1] = 0.0; }
-                mbar_wait(stg_full, tpar);
-                for (int u = warp; u < nblk * rs; u += WM) {
-                    const int blk = u / rs, part = u - blk * rs;
-                    const int g = blk / wvalid, wl = blk - g * wvalid;
-                    const int i_lo = (part * n) / rs, i_hi = ((part + 1) * n) / rs;
-                    const int gn = g * P.nb, cb = wl * n;
-                    const bool cplx = P.cplx != 0;
-                    // element T_ij = R + iI of the block, from the parked products C = Ltilde theta^T:
-                    //   real Ltilde:     R = C[i][re j],                   I = C[i][im j]
-                    //   complex Ltilde:  R = C[re i][re j] - C[im i][im j], I = C[re i][im j] + C[im i][re j]   (rows im i = n + i)
-                    auto elem = [&](const double *p, int row, int col, double &re, double &im) {
-                        const double *q = p + (row >> 1) * LD2 + (row & 1) * H + col;
-                        re = q[0]; im = q[planeoff];
-                        if (cplx) {
-                            const int r2 = row + n;
-                            const double *q2 = p + (r2 >> 1) * LD2 + (r2 & 1) * H + col;
-                            re -= q2[planeoff]; im += q2[0];
-                        }
-                    };
-                    double xr = 0.0, xi = 0.0, yr = 0.0, yi = 0.0, tr = 0.0, ti = 0.0;
-                    for (int j0 = 0; j0 < n; j0 += 32) {
-                        const int j = j0 + lane;
-                        if (j < n) {
-                            const double *blkp = staging + cb;
-                            if (part == 0) { double r, im; elem(blkp, gn + j, j, r, im); tr += r; ti += im; }
-                            int i = i_lo;
-                            for (; i + 1 < i_hi; i += 2) {                                          // two independent chains
-                                double a_r, a_i, b_r, b_i, c_r, c_i, d_r, d_i;
-                                elem(blkp, gn + i, j, a_r, a_i); elem(blkp, gn + j, i, b_r, b_i);            // T_ij, T_ji
-                                elem(blkp, gn + i + 1, j, c_r, c_i); elem(blkp, gn + j, i + 1, d_r, d_i);
-                                xr = fma(a_r, b_r, xr); yr = fma(c_r, d_r, yr);
-                                xr = fma(-a_i, b_i, xr); yr = fma(-c_i, d_i, yr);
-                                xi = fma(a_r, b_i, xi); yi = fma(c_r, d_i, yi);
-                            }
-                            if (i < i_hi) {
-                                double a_r, a_i, b_r, b_i;
-                                elem(blkp, gn + i, j, a_r, a_i); elem(blkp, gn + j, i, b_r, b_i);
-                                xr = fma(a_r, b_r, xr);
-                                xr = fma(-a_i, b_i, xr);
-                                xi = fma(a_r, b_i, xi);
-                            }
-                        }
-                    }
-                    xr = warp_sum(xr + yr); xi = warp_sum(xi + yi);
-                    if (part == 0) { tr = warp_sum(tr); ti = warp_sum(ti); }
-                    if (lane == 0) {
-                        if (part == 0) {
-                            double *tp = P.tbuf + ((long long)(w0 + wl) * P.n_gamma + g0 + g) * 2;
-                            tp[0] = tr; tp[1] = ti;
-                        }
-                        redp[(wl * K2_MAX_WM + warp) * 2] += xr;
-                        redp[(wl * K2_MAX_WM + warp) * 2 + 1] += 2.0 * xi;
-                    }
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(stg_free);
-                if (warp == WM - 1) {                    // the lightest warp adds the per-warp shares in a fixed order
-                    mbar_wait(stg_free, tpar);
-                    if (lane < wvalid) {
-                        double sr = 0.0, si = 0.0;
-                        for (int q = 0; q < WM; ++q) { sr += redp[(lane * K2_MAX_WM + q) * 2]; si += redp[(lane * K2_MAX_WM + q) * 2 + 1]; }
-                        double *xp = P.xpart + ((long long)rt * P.maxw + w0 + lane) * 2;
-                        xp[0] = sr; xp[1] = si;
-                    }
-                }
-            }
-            tpar ^= 1u;
-            rt += step_rt; ct += step_ct;
-            if (ct >= P.n_ct) { ct -= P.n_ct; ++rt; }
-        }
-    };
-    if (role == 0) run_tiles(std::integral_constant<int, 0>{});
-    else if (role == 1) run_tiles(std::integral_constant<int, 1>{});
-    else run_tiles(std::integral_constant<int, 2>{});
-}
-
-// ------------------------------------------------------------------------------------------------------------------
 // Force-bias GEMM (Eq. 24; Listing 3): xbar^gamma_w = sum_ip Ltilde^gamma_ip theta^w_ip.
 // Same operand ring and K loop as the exchange kernel, with the operands packed for n = 1 and k = (i, p): rows are
 // gamma (x Re/Im of Ltilde for a complex trial), columns are (plane, walker), every warp owns one 8-row strip and all NT
