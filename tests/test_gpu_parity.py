@@ -351,6 +351,34 @@ def test_host_entry_point_and_force_bias():
     le.close()
 
 
+@pytest.mark.parametrize("N,na,nb,ng,nw", [
+    (20, 5, 4, 23, 67),     # three blocks: first eighth of alpha (rounded up to whole K2 column tiles), rest of alpha, beta; ragged tail
+    (20, 0, 4, 23, 40),     # no alpha electrons: the blocks are cut from the beta spin
+    (20, 5, 0, 23, 33),     # no beta electrons
+    (33, 13, 11, 12, 19),   # two walkers per K2 column tile: block boundaries fall on tile boundaries
+])
+def test_host_entry_point_in_blocks_is_bit_identical_and_matches_oracle(N, na, nb, ng, nw):
+    """afqmc_local_energy_host copies the walkers in up to three blocks and runs K1 + K2 block by block on walker ranges
+    (include/afqmc.h): the result must equal afqmc_local_energy bit for bit, and the oracle to 1e-10."""
+    inp = _custom(900 + nw, N, na, nb, ng, nw)
+    le = _le(inp)
+    E, lo = gpu_energy(inp, le)
+    wh = torch.from_numpy(inp.walkers_packed()).pin_memory()
+    Eh, loh = le.local_energy_host(wh, nw)
+    assert np.array_equal(Eh.numpy().view(np.float64), E.view(np.float64))
+    assert np.array_equal(loh.numpy().view(np.float64), lo.view(np.float64))
+    Eh2, _ = le.local_energy_host(torch.from_numpy(inp.walkers_packed()), nw)            # pageable host memory
+    assert np.array_equal(Eh2.numpy().view(np.float64), E.view(np.float64))
+    idx = sorted({0, nw // 8, nw // 8 + 1, nw // 2, nw - 1})
+    Eo, loo = orc.local_energy_batch(inp, rung="O3", walkers=idx)
+    assert_parity(E[idx], lo[idx], Eo, loo)
+    fewer = max(1, nw // 3)                                                              # fewer walkers than capacity, host path
+    Ef, _ = le.local_energy_host(torch.from_numpy(inp.walkers_packed(list(range(fewer)))).pin_memory(), fewer)
+    Ed, _ = gpu_energy(inp, le, idx=list(range(fewer)))
+    assert np.array_equal(Ef.numpy().view(np.float64), Ed.view(np.float64))
+    le.close()
+
+
 @pytest.mark.parametrize("case", ["small", "ragged", "complex", "one_spin"])
 def test_force_bias_only_matches_oracle_and_energy_path(case):
     """Dedicated force-bias GEMM (afqmc_force_bias_only) against sum_pq G_pq L^gamma_pq from the full Green's
