@@ -95,6 +95,27 @@ def test_propagate_edge_shapes(N, na, nb, ng, nw, cx):
     _assert_step(inp, x, wts, dt, got)
 
 
+@pytest.mark.parametrize("N,na,nb,ng,nw", [
+    (12, 3, 2, 6, 160),     # one K9 row tile per walker: 148 walkers fill a round, the other 12 go in the finer-tiled launch
+    (170, 4, 3, 5, 80),     # two row tiles per walker (22 strips): 74 walkers in whole rounds, 6 walkers as 4 tiles of 6 strips
+])
+def test_propagate_batches_larger_than_one_round_of_ctas(N, na, nb, ng, nw):
+    """k9_apply runs one CTA per SM; batch items beyond whole rounds of the GPU go in a second launch with row tiles of
+    half the height (launch_k9 in csrc/afqmc.cu).  Walkers on both sides of that boundary against the oracle."""
+    inp = _custom(1300 + N, N, na, nb, ng, nw)
+    inp = Inputs(**{**inp.__dict__, "chol": inp.chol * 0.3})
+    x, wts = _fields(inp, 23)
+    dt = _converging_dt(inp, x)
+    got = _gpu_step(inp, x, wts, dt, order=40)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    per_item = (((N + 7) // 8) + 19) // 20
+    main_items = (per_item * nw // sms) * sms // per_item
+    assert 0 < main_items < nw
+    idx = sorted({0, main_items - 1, main_items, nw - 1})
+    sub = {k: v[idx] for k, v in got.items()}
+    _assert_step(inp, x, wts, dt, sub, walkers=idx)
+
+
 def test_propagate_truncated_series_and_batch_subsets_and_repeatability():
     """(i) a low Taylor order gives exactly the truncated series (checked against the oracle's matrices summed by
     hand), (ii) a subset of walkers on a larger handle, (iii) bit-identical repeats, (iv) zero fields at order 0 reduce
