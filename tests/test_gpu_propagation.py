@@ -9,6 +9,7 @@ import torch
 
 from gen import make_inputs
 from gen.configs import Inputs
+from oracle import afqmc_oracle as orc
 from oracle import propagation_oracle as prop
 from tests.test_gpu_parity import _custom, _le
 
@@ -114,6 +115,41 @@ def test_propagate_batches_larger_than_one_round_of_ctas(N, na, nb, ng, nw):
     idx = sorted({0, main_items - 1, main_items, nw - 1})
     sub = {k: v[idx] for k, v in got.items()}
     _assert_step(inp, x, wts, dt, sub, walkers=idx)
+
+
+def test_propagate_full_size_in_the_bench_configuration():
+    """Cu2O2-scale, all 256 walkers, the time step and Taylor order bench.py times (1e-4, 6): the propagated determinants and
+    the shift of sampled walkers -- the first, both sides of k9_apply's whole-rounds boundary (222 of 256 walkers on 148
+    SMs) and the last -- against the oracle's matrices with the series truncated at the same order, summed by hand."""
+    from tests.test_gpu_parity import _full_inputs
+    inp = _full_inputs("cu2o2")
+    x, wts = _fields(inp, 24)
+    dt, order = 1e-4, 6
+    got = _gpu_step(inp, x, wts, dt, order=order)
+    E = prop.expm_symmetric(-0.5 * dt * prop.one_body_shift(inp.h1e, inp.chol))
+    for w in (0, 221, 222, 255):
+        xbar = prop.force_bias_shift(inp.chol, inp.psi_a, inp.psi_b, inp.phi_a[w], inp.phi_b[w], dt)
+        assert np.max(np.abs(got["xbar"][w] - xbar)) <= RTOL * np.max(np.abs(xbar)), w
+        A = prop.hs_potential(inp.chol, dt, x[w] - xbar)
+        series, term = np.eye(inp.N, dtype=np.complex128), np.eye(inp.N, dtype=np.complex128)
+        for k in range(1, order + 1):
+            term = term @ A / k
+            series = series + term
+        new = {}
+        for key, phi in (("phi_a", inp.phi_a[w]), ("phi_b", inp.phi_b[w])):
+            new[key] = ref = E @ (series @ (E @ phi))
+            assert np.max(np.abs(got[key][w] - ref)) <= RTOL * np.max(np.abs(ref)), (w, key)
+        # overlap ratio and weight (Eq. 7-12) of the same truncated step; these synthetic Cholesky vectors are ~100x a
+        # molecule's, so the importance function may overflow exp(): then both sides must say inf
+        lo_old = complex(*orc.log_overlap(inp.psi_a, inp.psi_b, inp.phi_a[w], inp.phi_b[w]))
+        lo_new = complex(*orc.log_overlap(inp.psi_a, inp.psi_b, new["phi_a"], new["phi_b"]))
+        assert abs(got["lo"][w].real - lo_new.real) <= RTOL * max(1.0, abs(lo_new.real)), w
+        w_ref = orc.phaseless_weight_update(wts[w], lo_old, lo_new, x[w], xbar)
+        if np.isfinite(w_ref):
+            assert abs(got["weight"][w] - w_ref) <= 1e-8 * max(abs(w_ref), 1e-300), (w, got["weight"][w], w_ref)
+        else:
+            assert got["weight"][w] == w_ref, (w, got["weight"][w], w_ref)
+    assert not np.any(np.isnan(got["weight"])) and np.all(got["weight"] >= 0.0)
 
 
 def test_propagate_truncated_series_and_batch_subsets_and_repeatability():
