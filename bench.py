@@ -211,7 +211,7 @@ def main():
     trial = torch.from_numpy(inp.trial_packed()).to(dev)
     le = LocalEnergy(h1e, chol, trial, inp.N, inp.n_alpha, inp.n_beta, inp.n_gamma, inp.e0, nw)
     le.enable_force_bias(chol)          # operand of the dedicated force-bias GEMM (reported under "force_bias")
-    PROP_DT, PROP_ORDER = 0.0001, 6     # customary Taylor order; 1/50 of the paper's Cu2O2 time step
+    PROP_DT, PROP_ORDER = 0.00005, 6    # customary Taylor order; 1/100 of the paper's Cu2O2 time step
     # because the synthetic Cholesky vectors are ~100x a molecule's: at 0.005 the overlap ratio overflows exp()
     if not args.no_propagation:
         le.enable_propagation(h1e, chol, PROP_DT)
@@ -292,9 +292,8 @@ def main():
     # ---- one hybrid propagation step: K1, force bias, field GEMM, Taylor, K1, weights --
     prop = None
     if not args.no_propagation:
-        gen = torch.Generator(device=dev)
-        gen.manual_seed(1234 + rank)
-        xf = torch.randn((nw, inp.n_gamma), dtype=torch.float64, device=dev, generator=gen)
+        from paper_2209_04015_b200 import sample_fields
+        xf = sample_fields(1234, 0, nw, inp.n_gamma, first_walker=w_start, device=dev)     # Eq. 4's x, drawn before the timed region
         wts = torch.ones(nw, dtype=torch.float64, device=dev)
         wts_out, lo_out = torch.empty_like(wts), torch.empty(nw, dtype=torch.complex128, device=dev)
         wk = walkers.clone()

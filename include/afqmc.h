@@ -25,8 +25,10 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *   - Return value: AFQMC_OK or a negative error code; afqmc_last_error() gives the text.  Argument errors are
  *     detected before any work is enqueued.
- *   - Tuning override (benchmarks only; results do not depend on it): the environment variable
- *     AFQMC_K2_PIPELINE="k,s" forces K2's shared-memory ring to s stages of k DMMA k-steps each when that fits.
+ *   - Tuning overrides (benchmarks only; results do not depend on them): the environment variable
+ *     AFQMC_K2_PIPELINE="k,s" forces K2's shared-memory ring to s stages of k DMMA k-steps each when that fits;
+ *     AFQMC_K2_SHAPE="warps,ctas_per_sm,gammas_per_tile,walkers_per_tile" forces K2's CTA shape (0 = planner's choice
+ *     for the last two).  Both are read once per process.
  *   - A handle owns one set of workspaces: calls on the same handle must be ordered (one stream, or streams the
  *     caller has ordered with events); use one handle per concurrent stream.  Handles are independent of each other.
  *   - Requires compute capability 10.x (sm_100a); anything else returns AFQMC_ERR_ARCH.  There is no CPU path.
@@ -156,6 +158,18 @@ int afqmc_greens_function(afqmc_ctx *ctx, int spin, void *out, void *stream);
  */
 int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const void *xbar, const void *log_ovlp_old,
                             const void *log_ovlp_new, const double *weights_in, double *weights_out, void *stream);
+
+/*
+ * afqmc_sample_fields -- the auxiliary fields of one propagation step, x[w][gamma] ~ N(0, 1) (Eq. 4: "p(x) is
+ * the normal distribution").  The paper names no generator; this is a counter-based one (Philox4x32-10 + Box-Muller,
+ * DESIGN.md section 3 row 21; csrc/k10_fields.cuh states the exact mapping), so the call keeps no state:
+ *     x[w][2b], x[w][2b+1]  <-  Philox4x32-10(counter = (b, first_walker + w, step lo, step hi), key = (seed lo, seed hi))
+ * A walker's fields depend only on (seed, step, its global index first_walker + w, gamma): not on the batch, the rank or
+ * the launch.  Optional: afqmc_propagate takes x from any source.
+ *   x   device, float64 [n_walkers][n_gamma].   n_walkers, n_gamma >= 1, first_walker >= 0.   Enqueued on `stream`.
+ */
+int afqmc_sample_fields(unsigned long long seed, unsigned long long step, int first_walker, int n_walkers, int n_gamma,
+                        double *x, void *stream);
 
 /*
  * afqmc_enable_propagation / afqmc_propagate -- one step of the hybrid phaseless propagation for all walkers

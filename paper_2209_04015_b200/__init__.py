@@ -5,6 +5,6 @@ does not load the library; the first use does, and fails loudly if it has not be
 (``python -c "import __graft_entry__ as g; g.build()"``).  There is no CPU fallback.
 """
 from .binding import (AfqmcError, LocalEnergy, fp64_peak_tflops, library_path, load_library, phaseless_weights,
-                      plan)  # noqa: F401
+                      plan, sample_fields)  # noqa: F401
 from .build import build_library  # noqa: F401
 from .parallel import gather_walker_results, max_over_ranks, walker_shard  # noqa: F401

@@ -17,7 +17,7 @@ EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afq
            "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_phaseless_weights", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
            "afqmc_fp64_peak", "afqmc_plan", "afqmc_plan_trial", "afqmc_enable_propagation", "afqmc_propagate",
-           "afqmc_propagation_xbar", "afqmc_propagate_phase_ms"]
+           "afqmc_propagation_xbar", "afqmc_propagate_phase_ms", "afqmc_sample_fields"]
 
 
 class AfqmcError(RuntimeError):
@@ -55,6 +55,8 @@ def load_library():
     lib.afqmc_local_energy_host.restype = ip
     lib.afqmc_force_bias.argtypes = [vp, vp, vp]
     lib.afqmc_force_bias.restype = ip
+    lib.afqmc_sample_fields.argtypes = [C.c_ulonglong, C.c_ulonglong, ip, ip, ip, vp, vp]
+    lib.afqmc_sample_fields.restype = ip
     lib.afqmc_enable_force_bias.argtypes = [vp, vp, vp]
     lib.afqmc_enable_force_bias.restype = ip
     lib.afqmc_force_bias_only.argtypes = [vp, vp, ip, vp, vp]
@@ -134,6 +136,22 @@ def phaseless_weights(x, xbar, log_ovlp_old, log_ovlp_new, weights, out=None, st
                                      log_ovlp_new.data_ptr(), weights.data_ptr(), out.data_ptr(), _stream_ptr(stream))
     if rc != 0:
         raise AfqmcError(f"afqmc_phaseless_weights failed ({rc}): {lib.afqmc_last_error(None).decode()}")
+    return out
+
+
+def sample_fields(seed, step, n_walkers, n_gamma, first_walker=0, out=None, device=None, stream=None):
+    """afqmc_sample_fields: the auxiliary fields x ~ N(0, 1) of one propagation step (Eq. 4), float64 [n_walkers, n_gamma] on
+    the GPU, from the counter-based generator the header describes (no state: the same arguments give the same numbers)."""
+    _require_cuda()
+    lib = load_library()
+    if out is None:
+        out = torch.empty((n_walkers, n_gamma), dtype=torch.float64, device=device or "cuda")
+    if not (out.is_cuda and out.is_contiguous() and out.dtype == torch.float64) or out.numel() != n_walkers * n_gamma:
+        raise AfqmcError("sample_fields: out must be a contiguous CUDA float64 tensor of n_walkers * n_gamma elements")
+    rc = lib.afqmc_sample_fields(int(seed) & (2 ** 64 - 1), int(step) & (2 ** 64 - 1), int(first_walker), int(n_walkers), int(n_gamma),
+                                 out.data_ptr(), _stream_ptr(stream))
+    if rc != 0:
+        raise AfqmcError(f"afqmc_sample_fields failed ({rc}): {lib.afqmc_last_error(None).decode()}")
     return out
 
 

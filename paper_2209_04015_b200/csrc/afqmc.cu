@@ -23,6 +23,7 @@
 #include "k6_greens.cuh"
 #include "k7_phaseless.cuh"
 #include "k8_propagate.cuh"
+#include "k10_fields.cuh"
 
 using namespace afqmc;
 
@@ -812,6 +813,15 @@ int afqmc_phaseless_weights(int n_walkers, int n_gamma, const double *x, const v
     return AFQMC_OK;
 }
 
+int afqmc_sample_fields(unsigned long long seed, unsigned long long step, int first_walker, int n_walkers, int n_gamma, double *x,
+                        void *stream_) {
+    if (n_walkers < 1 || n_gamma < 1 || first_walker < 0 || !x) return fail(nullptr, AFQMC_ERR_ARG, "afqmc_sample_fields: bad argument");
+    const long long pairs = (long long)n_walkers * ((n_gamma + 1) / 2);
+    k10_sample_fields<<<(unsigned)((pairs + 255) / 256), 256, 0, (cudaStream_t)stream_>>>(seed, step, first_walker, n_walkers, n_gamma, x);
+    CU_TRY(nullptr, cudaGetLastError());
+    return AFQMC_OK;
+}
+
 int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *chol, double dt, void *stream_) {
     if (!ctx) return AFQMC_ERR_ARG;
     if (!h1e || !chol) return fail(ctx, AFQMC_ERR_ARG, "afqmc_enable_propagation: null pointer argument");
@@ -890,7 +900,7 @@ int afqmc_enable_propagation(afqmc_ctx *ctx, const double *h1e, const double *ch
     CU_TRY(ctx, cudaMalloc(&ctx->v_B, b_bytes));
     CU_TRY(ctx, cudaMemsetAsync(ctx->v_A, 0, a_bytes, stream));
     CU_TRY(ctx, cudaMemsetAsync(ctx->v_B, 0, b_bytes, stream));
-    if (ksteps > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_enable_propagation: n_gamma > 262140 is not supported");
+    if (ksteps > 65535 || N > 65535) return fail(ctx, AFQMC_ERR_UNSUPPORTED, "afqmc_enable_propagation: n_gamma > 262140 or N > 65535 is not supported");
     k8_pack_chol_vhs<<<dim3((N + 127) / 128, N, ksteps), 128, 0, stream>>>(chol, N, n_gamma, ctx->v_layA, ctx->v_A);
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 4 + 18 + nsq;

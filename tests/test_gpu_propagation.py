@@ -118,13 +118,13 @@ def test_propagate_batches_larger_than_one_round_of_ctas(N, na, nb, ng, nw):
 
 
 def test_propagate_full_size_in_the_bench_configuration():
-    """Cu2O2-scale, all 256 walkers, the time step and Taylor order bench.py times (1e-4, 6): the propagated determinants and
+    """Cu2O2-scale, all 256 walkers, the time step and Taylor order bench.py times (5e-5, 6): the propagated determinants and
     the shift of sampled walkers -- the first, both sides of k9_apply's whole-rounds boundary (222 of 256 walkers on 148
     SMs) and the last -- against the oracle's matrices with the series truncated at the same order, summed by hand."""
     from tests.test_gpu_parity import _full_inputs
     inp = _full_inputs("cu2o2")
     x, wts = _fields(inp, 24)
-    dt, order = 1e-4, 6
+    dt, order = 5e-5, 6
     got = _gpu_step(inp, x, wts, dt, order=order)
     E = prop.expm_symmetric(-0.5 * dt * prop.one_body_shift(inp.h1e, inp.chol))
     for w in (0, 221, 222, 255):
