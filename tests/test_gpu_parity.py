@@ -245,6 +245,31 @@ def test_two_live_handles_of_different_size_used_alternately():
     le_small.close()
 
 
+def test_two_handles_on_two_streams_running_concurrently():
+    """"Use one handle per concurrent stream" (include/afqmc.h): two handles, two non-default streams, launches
+    interleaved without any synchronisation in between; each must return exactly what it returns alone."""
+    inps = [make_inputs("small", n_walkers=24, n_gamma=60), _custom(77, 33, 13, 11, 40, 19)]
+    les = [_le(i) for i in inps]
+    wks = [torch.from_numpy(i.walkers_packed()).cuda() for i in inps]
+    alone = []
+    for le, i, wk in zip(les, inps, wks):
+        E, lo = le.local_energy(wk, i.n_walkers)
+        torch.cuda.synchronize()
+        alone.append((E.clone(), lo.clone()))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [[], []]
+    for rep in range(6):
+        for k in (0, 1):
+            with torch.cuda.stream(streams[k]):
+                outs[k].append(les[k].local_energy(wks[k], inps[k].n_walkers, stream=streams[k]))
+    torch.cuda.synchronize()
+    for k in (0, 1):
+        for E, lo in outs[k]:
+            assert torch.equal(E, alone[k][0]) and torch.equal(lo, alone[k][1])
+    for le in les:
+        le.close()
+
+
 def test_outputs_of_the_last_call_are_sized_by_the_library_not_the_caller():
     """force_bias / spin_squared / greens_function write results for the walkers of the LAST call; the
     binding sizes `out` from that and rejects a caller-supplied count or buffer that disagrees."""
