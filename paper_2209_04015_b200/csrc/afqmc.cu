@@ -329,12 +329,18 @@ int launch_k1(afqmc_ctx *ctx, const void *walkers, int n_walkers, bool with_fb, 
     const int nwl = count < 0 ? n_walkers : count, nsp = spin < 0 ? 2 : 1;
     const size_t k1s = std::max(ctx->sp[0].k1_smem, ctx->sp[1].k1_smem);
     const dim3 grid(nwl, nsp);
-    if (big) {
-        if (with_fb) k1_overlap_inverse_theta<true, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
-        else k1_overlap_inverse_theta<true, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    // n <= 32: four CTAs per SM; larger n: two per SM when the shared memory allows it (measured at medium, n = 40:
+    // 0.185 -> 0.130 ms), else one per SM with the whole register file (large, n = 50: 1.21 ms against 1.45 at 128 registers)
+    const int size = !big ? 0 : (2 * (k1s + 1024) <= 233472 ? 1 : 2);
+    if (size == 2) {
+        if (with_fb) k1_overlap_inverse_theta<2, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
+        else k1_overlap_inverse_theta<2, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    } else if (size == 1) {
+        if (with_fb) k1_overlap_inverse_theta<1, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
+        else k1_overlap_inverse_theta<1, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
     } else {
-        if (with_fb) k1_overlap_inverse_theta<false, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
-        else k1_overlap_inverse_theta<false, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+        if (with_fb) k1_overlap_inverse_theta<0, true><<<grid, K1_THREADS, k1s, stream>>>(p1);
+        else k1_overlap_inverse_theta<0, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
     }
     CU_TRY(ctx, cudaGetLastError());
     ctx->launches += 1;
@@ -533,10 +539,12 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
         }
         CR_TRY(allow_max_smem(fn));
     }
-    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<false, false>));
-    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<false, true>));
-    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<true, false>));
-    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<true, true>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<0, false>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<0, true>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<1, false>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<1, true>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<2, false>));
+    CR_TRY(allow_max_smem(k1_overlap_inverse_theta<2, true>));
     CR_TRY(allow_max_smem(k5_spin_squared));
     CR_TRY(allow_max_smem(k6_greens_function));
     CR_TRY(cudaMalloc(&c->e1, (size_t)2 * max_walkers * 16));

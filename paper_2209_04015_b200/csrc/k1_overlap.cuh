@@ -304,9 +304,11 @@ __device__ unsigned long long g_k1_clocks[8];
 #define K1_MARK(i) do { } while (0)
 #endif
 
-// BIG = false: n <= 32 (<= 4 output tiles per warp and pass, four CTAs per SM); BIG = true: n <= 64.
-template <bool BIG, bool WITH_FB>
-__global__ void __launch_bounds__(K1_THREADS, BIG ? 1 : 4) k1_overlap_inverse_theta(K1Params P) {
+// SIZE 0: n <= 32 (<= 4 output tiles per warp and pass, 64 registers, four CTAs per SM); SIZE 1: n <= 64 with a shared-
+// memory footprint that lets two CTAs share an SM (128 registers); SIZE 2: n <= 64, one CTA per SM (all registers).
+template <int SIZE, bool WITH_FB>
+__global__ void __launch_bounds__(K1_THREADS, SIZE == 0 ? 4 : SIZE == 1 ? 2 : 1) k1_overlap_inverse_theta(K1Params P) {
+    constexpr bool BIG = SIZE > 0;
     constexpr int MAXT_S = BIG ? 16 : 4;     // S pass: tiles per warp
     constexpr int MAXT_T = BIG ? 8 : 4;      // theta pass: column blocks per warp
     const int w = blockIdx.x + P.w0, sp = blockIdx.y + P.spin0;
