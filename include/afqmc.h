@@ -51,7 +51,7 @@ enum {
     AFQMC_ERR_UNSUPPORTED = -5  /* valid input the library does not handle yet (n_sigma > 64)           */
 };
 
-#define AFQMC_MAX_NOCC 64 /* largest n_sigma supported (shared-memory LU and register-tile limits) */
+#define AFQMC_MAX_NOCC 64 /* largest n_sigma supported (shared-memory inversion and register-tile limits) */
 
 /*
  * afqmc_create -- one-time setup for a Hamiltonian and trial (Eq. 21).
@@ -74,7 +74,7 @@ int afqmc_create(const double *h1e, const double *chol, const void *trial, int N
                  int n_gamma, double e0, int max_walkers, void *stream, afqmc_ctx **out);
 
 /*
- * afqmc_local_energy -- the hot path: kernels K1 (overlap, LU, inverse, theta, E1), K2 (fused exchange +
+ * afqmc_local_energy -- the hot path: kernels K1 (overlap, determinant, inverse, theta, E1), K2 (fused exchange +
  * Coulomb traces, once per spin) and K3 (assembly), all enqueued on `stream`; returns without synchronising.
  *   walkers       device, complex128: alpha block [n_walkers][N][n_alpha] then beta block
  *                 [n_walkers][N][n_beta]  ("Nwalkers x M x N").  Need not be orthonormal.
