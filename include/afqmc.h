@@ -218,6 +218,29 @@ int afqmc_propagate(afqmc_ctx *ctx, void *walkers, int n_walkers, const double *
 int afqmc_propagation_xbar(afqmc_ctx *ctx, void *out, void *stream);
 int afqmc_propagate_phase_ms(afqmc_ctx *ctx, float ms[5]);
 
+/*
+ * afqmc_log_overlap_static -- the log-overlaps alone, from an entry point that ALLOCATES NOTHING: no handle, no cudaMalloc /
+ * cudaFree, no allocating library routine, no host synchronisation.  For callers that cannot allocate: code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it.
+ *     out_overlaps[w] = (log|<psi_T|phi_w>|, arg <psi_T|phi_w>),   <psi_T|phi_w> = det(psi_alpha^dagger phi_alpha,w) det(psi_beta^dagger phi_beta,w)
+ *                                                                                   PAPER.md:143 (Eq. 16), 146-150
+ * computed by kernel K1 as afqmc_local_energy runs it (same values as that call's out_overlaps).  Its scratch -- the trial
+ * packed for the tensor cores, the theta K1 writes as a by-product, per-walker partial results -- lives in ONE file-scope
+ * device array of AFQMC_STATIC_SCRATCH_BYTES that every GPU holds from the moment it loads the library until the process
+ * exits.  Sizes that need more return AFQMC_ERR_UNSUPPORTED with the byte counts in the message:
+ *     8 n_max N + 16 sum_sigma N n_sigma + 16 n_walkers sum_sigma N n_sigma (+ padding to tiles of 8 / 4 / 32) + 64 n_walkers  bytes,
+ * e.g. N = 290, n_alpha = n_beta = 26: up to 62 walkers per call; N = 100, n = 20: up to 260; N = 500, n = 50: up to 18.
+ *   trial         device, complex128, layout of afqmc_create (read on every call: no state is kept between calls)
+ *   walkers       device, complex128, layout of afqmc_local_energy;  n_walkers >= 1
+ *   out_overlaps  device, complex128 [n_walkers]
+ * Enqueued on `stream`, returns without synchronising.  ALL calls, from all threads and streams, share the one array (it
+ * keeps the last call's contents; the call clears what must start at zero): calls that overlap on the GPU -- different
+ * streams without an ordering between them -- race.  Order them, or use handles (afqmc_create) instead.
+ */
+#define AFQMC_STATIC_SCRATCH_BYTES 16777216 /* 16 MiB per GPU that loads the library */
+int afqmc_log_overlap_static(const void *trial, const void *walkers, int N, int n_alpha, int n_beta, int n_walkers,
+                             void *out_overlaps, void *stream);
+
 /* Frees the handle and every internal buffer.  NULL is allowed. */
 void afqmc_destroy(afqmc_ctx *ctx);
 

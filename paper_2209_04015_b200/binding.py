@@ -17,7 +17,7 @@ EXPORTS = ["afqmc_create", "afqmc_local_energy", "afqmc_local_energy_host", "afq
            "afqmc_enable_force_bias", "afqmc_force_bias_only", "afqmc_spin_squared", "afqmc_greens_function", "afqmc_phaseless_weights", "afqmc_destroy",
            "afqmc_last_error", "afqmc_get_info", "afqmc_set_profiling", "afqmc_last_kernel_ms", "afqmc_mean_kernel_ms",
            "afqmc_fp64_peak", "afqmc_plan", "afqmc_plan_trial", "afqmc_enable_propagation", "afqmc_propagate",
-           "afqmc_propagation_xbar", "afqmc_propagate_phase_ms", "afqmc_sample_fields"]
+           "afqmc_propagation_xbar", "afqmc_propagate_phase_ms", "afqmc_sample_fields", "afqmc_log_overlap_static"]
 
 
 class AfqmcError(RuntimeError):
@@ -57,6 +57,8 @@ def load_library():
     lib.afqmc_force_bias.restype = ip
     lib.afqmc_sample_fields.argtypes = [C.c_ulonglong, C.c_ulonglong, ip, ip, ip, vp, vp]
     lib.afqmc_sample_fields.restype = ip
+    lib.afqmc_log_overlap_static.argtypes = [vp, vp, ip, ip, ip, ip, vp, vp]
+    lib.afqmc_log_overlap_static.restype = ip
     lib.afqmc_enable_force_bias.argtypes = [vp, vp, vp]
     lib.afqmc_enable_force_bias.restype = ip
     lib.afqmc_force_bias_only.argtypes = [vp, vp, ip, vp, vp]
@@ -152,6 +154,25 @@ def sample_fields(seed, step, n_walkers, n_gamma, first_walker=0, out=None, devi
                                  out.data_ptr(), _stream_ptr(stream))
     if rc != 0:
         raise AfqmcError(f"afqmc_sample_fields failed ({rc}): {lib.afqmc_last_error(None).decode()}")
+    return out
+
+
+def log_overlap_static(trial, walkers, N, n_alpha, n_beta, n_walkers, out=None, stream=None):
+    """afqmc_log_overlap_static: log-overlaps [n_walkers] complex128 without a handle and without any allocation inside the
+    library (pass ``out`` to keep this wrapper allocation-free too).  Sizes beyond the library's static scratch raise."""
+    _require_cuda()
+    lib = load_library()
+    for t, cnt in ((trial, N * (n_alpha + n_beta)), (walkers, n_walkers * N * (n_alpha + n_beta))):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.complex128) or t.numel() != cnt:
+            raise AfqmcError("log_overlap_static: trial / walkers must be contiguous CUDA complex128 tensors of the documented sizes")
+    if out is None:
+        out = torch.empty(n_walkers, dtype=torch.complex128, device=walkers.device)
+    if not (out.is_cuda and out.is_contiguous() and out.dtype == torch.complex128) or out.numel() != n_walkers:
+        raise AfqmcError("log_overlap_static: out must be a contiguous CUDA complex128 tensor of n_walkers elements")
+    rc = lib.afqmc_log_overlap_static(trial.data_ptr(), walkers.data_ptr(), int(N), int(n_alpha), int(n_beta), int(n_walkers),
+                                      out.data_ptr(), _stream_ptr(stream))
+    if rc != 0:
+        raise AfqmcError(f"afqmc_log_overlap_static failed ({rc}): {lib.afqmc_last_error(None).decode()}")
     return out
 
 

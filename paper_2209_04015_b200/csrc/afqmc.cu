@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -24,6 +25,7 @@
 #include "k7_phaseless.cuh"
 #include "k8_propagate.cuh"
 #include "k10_fields.cuh"
+#include "k11_pack_trial.cuh"
 
 using namespace afqmc;
 
@@ -1159,3 +1161,117 @@ int afqmc_k1_phase_clocks(long long out[8]) {
 #endif
 
 }  // extern "C"
+
+// ---- afqmc_log_overlap_static: an entry point that allocates nothing ------------------------------------------------------
+// Its scratch (psi^T fragment planes, a zero block standing in for htilde, the packed theta K1 writes, K1's per-walker
+// outputs) lives in this file-scope array: every GPU that loads the library holds AFQMC_STATIC_SCRATCH_BYTES of it until
+// the process exits.  In host code the array's name is only a host-side stand-in; the device address comes from
+// cudaGetSymbolAddress, once per device (static_scratch_for_current_device).
+static __device__ __align__(256) unsigned char g_static_scratch[AFQMC_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char *g_static_ptr[kMaxDevices] = {};
+
+// Device address of g_static_scratch on the current device; first use on a device also opts the K1 kernels in to their
+// dynamic shared memory there.  No allocation.
+int static_scratch_for_current_device(unsigned char **out) {
+    int dev = 0;
+    CU_TRY(nullptr, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_log_overlap_static: device ordinal %d >= %d", dev, kMaxDevices);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        unsigned char *ptr = nullptr;
+        CU_TRY(nullptr, cudaGetSymbolAddress((void **)&ptr, g_static_scratch));
+        if (!ptr) return fail(nullptr, AFQMC_ERR_CUDA, "afqmc_log_overlap_static: cudaGetSymbolAddress returned a null address");
+        CU_TRY(nullptr, allow_max_smem(k1_overlap_inverse_theta<0, false>));
+        CU_TRY(nullptr, allow_max_smem(k1_overlap_inverse_theta<1, false>));
+        CU_TRY(nullptr, allow_max_smem(k1_overlap_inverse_theta<2, false>));
+        g_static_ptr[dev] = ptr;
+    }
+    *out = g_static_ptr[dev];
+    return AFQMC_OK;
+}
+
+size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+}  // namespace
+
+extern "C" int afqmc_log_overlap_static(const void *trial, const void *walkers, int N, int n_alpha, int n_beta, int n_walkers,
+                                        void *out_overlaps, void *stream_) {
+    if (!trial || !walkers || !out_overlaps) return fail(nullptr, AFQMC_ERR_ARG, "afqmc_log_overlap_static: null pointer argument");
+    if (N < 1 || n_walkers < 1 || n_alpha < 0 || n_beta < 0 || n_alpha > N || n_beta > N || n_alpha + n_beta < 1)
+        return fail(nullptr, AFQMC_ERR_ARG, "afqmc_log_overlap_static: size out of range (N=%d n_alpha=%d n_beta=%d n_walkers=%d)", N, n_alpha,
+                    n_beta, n_walkers);
+    if (n_alpha > AFQMC_MAX_NOCC || n_beta > AFQMC_MAX_NOCC)
+        return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "afqmc_log_overlap_static: n_sigma > %d is not supported", AFQMC_MAX_NOCC);
+    if (int rc = check_arch(nullptr, nullptr)) return rc;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int ns[2] = {n_alpha, n_beta};
+    const int nmax = std::max(n_alpha, n_beta), ksteps = (N + 3) / 4, kpad = 8 * ((N + K1_ROWS - 1) / K1_ROWS);
+
+    // ---- carve the scratch: [zero block n_max x N][per spin: Re plane, Im plane][per spin: theta][e1][logdet] -------------------
+    size_t off = 0, plane_bytes[2], theta_bytes[2], plane_off[2][2], theta_off[2];
+    const size_t zero_off = off;
+    off += align256((size_t)nmax * N * 8);
+    for (int s = 0; s < 2; ++s) {
+        plane_bytes[s] = (size_t)kpad * ((ns[s] + 7) / 8) * 32 * 8;
+        for (int pl = 0; pl < 2; ++pl) { plane_off[s][pl] = off; off += align256(plane_bytes[s]); }
+    }
+    const size_t clear_bytes = off;                                   // everything up to here must start at zero
+    for (int s = 0; s < 2; ++s) {
+        theta_bytes[s] = (size_t)n_walkers * ((2 * ns[s] + 7) / 8) * ksteps * 32 * 8;
+        theta_off[s] = off; off += align256(theta_bytes[s]);
+    }
+    const size_t e1_off = off; off += align256((size_t)2 * n_walkers * 16);
+    const size_t ld_off = off; off += align256((size_t)2 * n_walkers * 16);
+    if (off > (size_t)AFQMC_STATIC_SCRATCH_BYTES)
+        return fail(nullptr, AFQMC_ERR_UNSUPPORTED,
+                    "afqmc_log_overlap_static: N=%d n_alpha=%d n_beta=%d n_walkers=%d needs %zu bytes of scratch, the static array holds %d "
+                    "(use afqmc_create / afqmc_local_energy for larger batches)", N, n_alpha, n_beta, n_walkers, off, AFQMC_STATIC_SCRATCH_BYTES);
+    unsigned char *base = nullptr;
+    if (int rc = static_scratch_for_current_device(&base)) return rc;
+
+    // ---- the array keeps the last call's contents: clear the zero block and the fragment planes (their padding) -----------------
+    CU_TRY(nullptr, cudaMemsetAsync(base, 0, clear_bytes, stream));
+    size_t toff = 0;
+    for (int s = 0; s < 2; ++s) {
+        if (ns[s] == 0) continue;
+        k11_pack_trial<<<(N * ns[s] + 255) / 256, 256, 0, stream>>>(reinterpret_cast<const double2 *>(trial) + toff, N, ns[s],
+                                                                   reinterpret_cast<double *>(base + plane_off[s][0]),
+                                                                   reinterpret_cast<double *>(base + plane_off[s][1]));
+        CU_TRY(nullptr, cudaGetLastError());
+        toff += (size_t)N * ns[s];
+    }
+
+    // ---- K1 as it stands (k1_overlap.cuh), complex-trial path (an all-zero Im plane adds exact zeros), theta into the scratch ----
+    K1Params p1{};
+    p1.walkers = reinterpret_cast<const double2 *>(walkers);
+    p1.n_walkers = n_walkers; p1.N = N; p1.maxw = n_walkers; p1.spin0 = 0; p1.w0 = 0;
+    p1.spin_off[0] = 0; p1.spin_off[1] = (long long)n_walkers * N * n_alpha;
+    size_t k1s = 0;
+    for (int s = 0; s < 2; ++s) {
+        p1.n[s] = ns[s];
+        if (ns[s] == 0) continue;
+        p1.psiA[s] = reinterpret_cast<const double *>(base + plane_off[s][0]);
+        p1.psiA_im[s] = reinterpret_cast<const double *>(base + plane_off[s][1]);
+        p1.ht[s] = p1.ht_im[s] = reinterpret_cast<const double *>(base + zero_off);
+        p1.thetaB[s] = reinterpret_cast<double *>(base + theta_off[s]);
+        const int strips = (2 * ns[s] + 7) / 8;
+        p1.layB[s] = OperandLayout{ns[s], strips, ksteps, 1, (long long)strips * ksteps * 32};      // one walker per tile
+        k1s = std::max(k1s, (size_t)k1_layout(ns[s], true).total);
+    }
+    p1.e1 = reinterpret_cast<double *>(base + e1_off);
+    p1.logdet = reinterpret_cast<double *>(base + ld_off);
+    const int size = nmax <= 32 ? 0 : (2 * (k1s + 1024) <= 233472 ? 1 : 2);
+    const dim3 grid(n_walkers, 2);
+    if (size == 2) k1_overlap_inverse_theta<2, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    else if (size == 1) k1_overlap_inverse_theta<1, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    else k1_overlap_inverse_theta<0, false><<<grid, K1_THREADS, k1s, stream>>>(p1);
+    CU_TRY(nullptr, cudaGetLastError());
+    k8_log_overlap<<<(n_walkers + 127) / 128, 128, 0, stream>>>(n_walkers, n_walkers, n_alpha, n_beta, p1.logdet, reinterpret_cast<double *>(out_overlaps));
+    CU_TRY(nullptr, cudaGetLastError());
+    return AFQMC_OK;
+}
