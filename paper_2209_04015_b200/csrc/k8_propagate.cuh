@@ -183,8 +183,10 @@ __global__ void k8_set_diagonal(double *M, int N, int ld, double s) {
 //        (Mre + i Mim) T = Mre T + Mim (i T),   (i T)[q][2m] = -T[q][2m+1],  (i T)[q][2m+1] = T[q][2m],
 //        so one accumulator set takes both products; the C fragment of DMMA.8x8x4 holds (re, im) of one complex entry.
 // Tiling: grid (row tiles, column groups of <= 104 columns, batch), 12 warps, warp w owns strips w and w + 12 of the row
-// tile (rt_strips <= 24) and all <= 13 column blocks (K2's register shape: 2 x 13 accumulator tiles per warp); the q range is staged through shared memory in chunks of 16 by
-// 8-byte cp.async, double buffered.  Pitches 20 / 116 doubles (= 4 mod 16) make the fragment loads conflict free.
+// tile (rt_strips <= 20) and all <= 13 column blocks (K2's register shape: 2 x 13 accumulator tiles per warp); the q range
+// is staged through shared memory in chunks of 16 by 16-byte (8-byte for odd pitches) cp.async into a ring of three
+// stages, one CTA barrier per chunk.  Pitches 20 / 116 doubles (= 4 mod 16) make the fragment loads conflict free.
+// Optional Add_b: Out_b = Add_b + alpha M_b In_b (a Horner step of the Taylor series).
 constexpr int K9_THREADS = 384;
 constexpr int K9_WARPS = K9_THREADS / 32;
 constexpr int K9_KC = 16;             // q per chunk = 4 DMMA k-steps
@@ -205,7 +207,7 @@ struct K9Params {
     long long io_batch_stride;
     int ld;                          // even
     int N, C;                        // M is N x N; In has C real columns in use
-    int rt_strips;                   // strips per row tile (<= 24)
+    int rt_strips;                   // strips per row tile (<= 20)
     int cg_blocks;                   // 8-column blocks per column group (<= K9_NT); grid.y groups cover C
     double alpha;
 };
