@@ -187,6 +187,12 @@ __global__ void k8_set_diagonal(double *M, int N, int ld, double s) {
 // is staged through shared memory in chunks of 16 by 16-byte (8-byte for odd pitches) cp.async into a ring of three
 // stages, one CTA barrier per chunk.  Pitches 20 / 116 doubles (= 4 mod 16) make the fragment loads conflict free.
 // Optional Add_b: Out_b = Add_b + alpha M_b In_b (a Horner step of the Taylor series).
+// Timing ablations (results are WRONG, only the time counts; AFQMC_NVCC_EXTRA=-DAFQMC_K9_ABLATE=n, see build.py):
+//   1  only the first two chunks are ever copied (no global loads, no copy code in the chunk loop)
+//   2  as 1, and no CTA barrier in the chunk loop            3  as 2, and no epilogue (accumulators kept alive by a dead store)
+#ifndef AFQMC_K9_ABLATE
+#define AFQMC_K9_ABLATE 0
+#endif
 constexpr int K9_THREADS = 384;
 constexpr int K9_WARPS = K9_THREADS / 32;
 constexpr int K9_KC = 16;             // q per chunk = 4 DMMA k-steps
@@ -221,6 +227,10 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N_>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_) : "memory"); }
 
+__device__ __forceinline__ void k9_cp16(uint32_t dst_smem, const void *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(dst_smem), "l"(src) : "memory");
+}
+
 __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads x 168 registers = the register file
     extern __shared__ __align__(16) unsigned char k9_smem[];
     double *sS = reinterpret_cast<double *>(k9_smem);                          // [3 stages]{ A [2 planes][160][20], B [16][116] }
@@ -253,7 +263,44 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
         b_c[j] = (e - (e / bpieces) * bpieces) * 2;
     }
 
-    auto load_chunk = [&](int stage, int q0) {
+    // The same duties for a chunk that lies wholly inside [0, N) when the 16-byte pieces apply: source offsets (elements,
+    // relative to the plane / to In) and shared-window destinations of stage 0, computed once; a copy is then one 64-bit
+    // add and the instruction itself (the general path below spends ~30 instructions per copy on bounds and addresses,
+    // measured as 16 % of the kernel).  Rows / columns beyond the tile's valid range are skipped: what the tensor cores
+    // compute from the stale shared memory there lands in accumulator rows / columns that are never stored.
+    const uint32_t sS_u = smem_u32(sS);
+    int fa_off[4], fb_off[3];
+    uint32_t fa_dst[4], fb_dst[3];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int r = a_r0 + k * 48;
+        fa_off[k] = (avec && r < rows) ? (row0 + r) * P.ldm + a_piece : -1;
+        fa_dst[k] = sS_u + (uint32_t)((r * K9_APITCH + a_piece) * 8);
+    }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        fb_off[j] = (b_k[j] >= 0 && b_c[j] < ncols) ? b_k[j] * P.ld + col0 + b_c[j] : -1;
+        fb_dst[j] = sS_u + (uint32_t)((2 * K9_MAXROWS * K9_APITCH + b_k[j] * K9_BPITCH + b_c[j]) * 8);
+    }
+    auto load_chunk_fast = [&](int stage, int q0) {
+        const uint32_t st = (uint32_t)stage * (K9_STAGE_DOUBLES * 8);
+        const double *mre = Mre + q0, *in = In + (long long)q0 * P.ld;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (fa_off[k] >= 0) k9_cp16(fa_dst[k] + st, mre + fa_off[k]);
+        if (cplx) {
+            const double *mim = Mim + q0;
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (fa_off[k] >= 0) k9_cp16(fa_dst[k] + st + K9_MAXROWS * K9_APITCH * 8, mim + fa_off[k]);
+        }
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+            if (fb_off[j] >= 0) k9_cp16(fb_dst[j] + st, in + fb_off[j]);
+        cp_async_commit();
+    };
+
+    auto load_chunk_any = [&](int stage, int q0) {
         double *a = sS + stage * K9_STAGE_DOUBLES;
         double *bb = a + 2 * K9_MAXROWS * K9_APITCH;
         const int qa = q0 + a_piece;
@@ -278,6 +325,10 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
         }
         cp_async_commit();
     };
+    auto load_chunk = [&](int stage, int q0) {
+        if (avec && q0 + K9_KC <= N) load_chunk_fast(stage, q0);
+        else load_chunk_any(stage, q0);
+    };
 
     double acc[2][K9_NT][2];
 #pragma unroll
@@ -297,7 +348,9 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
     for (int ch = 0; ch < nchunks; ++ch) {
         if (ch + 1 < nchunks) cp_async_wait<1>();
         else cp_async_wait<0>();
+#if AFQMC_K9_ABLATE < 2
         __syncthreads();
+#endif
         const double *a = sS + (ch % K9_STAGES) * K9_STAGE_DOUBLES;
         const double *bb = a + 2 * K9_MAXROWS * K9_APITCH;
         // A predicated-off DMMA still occupies the tensor pipe, so the strip count (MM) and the complex second product are
@@ -342,8 +395,21 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
             if (cplx) chunk_mma(std::integral_constant<int, 1>{}, std::true_type{});
             else chunk_mma(std::integral_constant<int, 1>{}, std::false_type{});
         }
+#if AFQMC_K9_ABLATE == 0
         if (ch + 2 < nchunks) load_chunk((ch + 2) % K9_STAGES, (ch + 2) * K9_KC);
+#endif
     }
+#if AFQMC_K9_ABLATE >= 3
+    {
+        double keep = 0.0;
+#pragma unroll
+        for (int m = 0; m < 2; ++m)
+#pragma unroll
+            for (int q = 0; q < K9_NT; ++q) keep += acc[m][q][0] + acc[m][q][1];
+        if (keep == 1.2345678e300) P.Out[0] = keep;
+        return;
+    }
+#endif
 
     double *Out = P.Out + (long long)b * P.io_batch_stride;
     double *Sum = P.Sum ? P.Sum + (long long)b * P.io_batch_stride : nullptr;
@@ -353,21 +419,28 @@ __global__ void __maxnreg__(168) k9_apply(const K9Params P) {     // 384 threads
         if (m >= my_mt) continue;
         const int r = (warp + K9_WARPS * m) * 8 + fr;
         if (r >= rows) continue;
+        const long long off0 = (long long)(row0 + r) * P.ld + col0 + 2 * fk;   // ld is even and C is even or padded: (c, c+1) stay inside the row
+        if (Add) {              // all loads of the strip first (the stores below may alias them as far as the compiler knows)
+            double2 t[K9_NT];
+#pragma unroll
+            for (int q = 0; q < K9_NT; ++q)
+                if (q < nt && q * 8 + 2 * fk < ncols) t[q] = __ldg(reinterpret_cast<const double2 *>(Add + off0 + q * 8));
+#pragma unroll
+            for (int q = 0; q < K9_NT; ++q)
+                if (q < nt && q * 8 + 2 * fk < ncols) { acc[m][q][0] = fma(P.alpha, acc[m][q][0], t[q].x); acc[m][q][1] = fma(P.alpha, acc[m][q][1], t[q].y); }
+        } else {
+#pragma unroll
+            for (int q = 0; q < K9_NT; ++q) { acc[m][q][0] *= P.alpha; acc[m][q][1] *= P.alpha; }
+        }
 #pragma unroll
         for (int q = 0; q < K9_NT; ++q) {
-            const int c = q * 8 + 2 * fk;
-            if (q < nt && c < ncols) {                                          // ld is even and C is even or padded: (c, c+1) stay inside the row
-                const long long off = (long long)(row0 + r) * P.ld + col0 + c;
-                double2 v = make_double2(P.alpha * acc[m][q][0], P.alpha * acc[m][q][1]);
-                if (Add) {
-                    const double2 t0 = *reinterpret_cast<const double2 *>(Add + off);
-                    v.x += t0.x; v.y += t0.y;
-                }
-                *reinterpret_cast<double2 *>(Out + off) = v;
+            if (q < nt && q * 8 + 2 * fk < ncols) {
+                const double2 v = make_double2(acc[m][q][0], acc[m][q][1]);
+                *reinterpret_cast<double2 *>(Out + off0 + q * 8) = v;
                 if (Sum) {
-                    double2 s = *reinterpret_cast<double2 *>(Sum + off);
+                    double2 s = *reinterpret_cast<double2 *>(Sum + off0 + q * 8);
                     s.x += v.x; s.y += v.y;
-                    *reinterpret_cast<double2 *>(Sum + off) = s;
+                    *reinterpret_cast<double2 *>(Sum + off0 + q * 8) = s;
                 }
             }
         }
