@@ -56,3 +56,41 @@ def test_local_energy_replayed_from_a_cuda_graph_is_bit_identical(name, nw):
     t_graph = timed(graph.replay)
     print(f"{name}: {t_direct:.1f} us per step with direct launches, {t_graph:.1f} us replayed from a CUDA graph")
     le.close()
+
+
+def test_force_bias_only_and_propagate_replayed_from_cuda_graphs():
+    from paper_2209_04015_b200 import sample_fields
+    inp = make_inputs("small", n_walkers=9, n_gamma=50)
+    nw, dt = inp.n_walkers, 1e-4
+    le = _le(inp)
+    chol = torch.from_numpy(inp.chol).cuda()
+    le.enable_propagation(torch.from_numpy(inp.h1e).cuda(), chol, dt)          # also enables the force-bias path
+    wk0 = torch.from_numpy(inp.walkers_packed()).cuda()
+    x = sample_fields(5, 0, nw, inp.n_gamma)
+    wts = torch.ones(nw, dtype=torch.float64, device="cuda")
+
+    fb = torch.empty((nw, inp.n_gamma), dtype=torch.complex128, device="cuda")
+    le.force_bias_only(wk0, nw, fb)
+    torch.cuda.synchronize()
+    fb_direct = fb.clone()
+    g1 = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g1):
+        le.force_bias_only(wk0, nw, fb)
+    fb.zero_()
+    g1.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(fb, fb_direct)
+
+    wk = wk0.clone()
+    w_out, lo_out = torch.empty_like(wts), torch.empty(nw, dtype=torch.complex128, device="cuda")
+    le.propagate(wk, nw, x, wts, 6, w_out, lo_out)                              # direct step on a copy
+    torch.cuda.synchronize()
+    ref = (wk.clone(), w_out.clone(), lo_out.clone())
+    g2 = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g2):
+        le.propagate(wk, nw, x, wts, 6, w_out, lo_out)
+    wk.copy_(wk0); w_out.zero_(); lo_out.zero_()
+    g2.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(wk, ref[0]) and torch.equal(w_out, ref[1]) and torch.equal(lo_out, ref[2])
+    le.close()
