@@ -39,7 +39,6 @@ struct SpinCfg {
     int n = 0;
     int MT = 0, NT = 0, WM = 0, gT = 0, wT = 0, strips = 0, ksc = 0, nchunks = 0, nstages = 0, H = 0, LD2 = 0;
     int n_rt = 0, n_ct_max = 0;
-    int gH = 0, stg_strips = 0;                   // two-half epilogue: gamma blocks of the first half, strips of the staging buffer
     int ctas_per_sm = 1;                          // persistent K2 CTAs per SM (2: two half-size CTAs, epilogues overlap K loops)
     size_t k2_smem = 0, k1_smem = 0;
     OperandLayout layA{}, layB{};
@@ -142,19 +141,18 @@ void k2_staging_shape(int NT, int &H, int &LD2) {
     while (LD2 % 16 != 1) ++LD2;
 }
 
-// stg_strips: strips the staging buffer holds (the whole tile, or the larger half of a two-half epilogue); 0 = strips.
-size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages, int stg_strips = 0) {
+size_t k2_smem_bytes(int strips, int NT, int ksc, int nstages) {
     const size_t stage = (size_t)ksc * (strips + NT) * 256;
     int H = 0, LD2 = 0;
     k2_staging_shape(NT, H, LD2);
-    return nstages * stage + (size_t)(stg_strips > 0 ? stg_strips : strips) * 4 * LD2 * 8 + (size_t)2 * K2_MAX_WT * K2_MAX_WM * 16 + (size_t)(2 * nstages + 2) * 8 + 16;
+    return nstages * stage + (size_t)strips * 4 * LD2 * 8 + (size_t)2 * K2_MAX_WT * K2_MAX_WM * 16 + (size_t)(2 * nstages + 2) * 8 + 16;
 }
 
 // Pipeline shape for a tile: k-steps per chunk and ring depth that fit beside the whole-tile staging buffer.
-bool choose_pipeline(int strips, int NT, int ksteps, size_t budget, int &ksc, int &nst, int stg_strips = 0) {
+bool choose_pipeline(int strips, int NT, int ksteps, size_t budget, int &ksc, int &nst) {
     if (const PipelineOverride &ov = pipeline_override(); ov.set) {
         const int kc = ov.ksc, s = ov.stages;
-        if (kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 && k2_smem_bytes(strips, NT, kc, s, stg_strips) <= budget) {
+        if (kc >= 1 && kc <= ksteps && s >= 2 && s <= 16 && k2_smem_bytes(strips, NT, kc, s) <= budget) {
             ksc = kc; nst = s;
             return true;
         }
@@ -165,7 +163,7 @@ bool choose_pipeline(int strips, int NT, int ksteps, size_t budget, int &ksc, in
     for (int s = 2; s <= 5; ++s) {
         for (int kc = std::min(12, std::max(2, ksteps / 10)); kc >= 1; --kc) {   // short K loops want short chunks (tile start-up)
             if (kc > ksteps) continue;
-            if (k2_smem_bytes(strips, NT, kc, s, stg_strips) > budget) continue;
+            if (k2_smem_bytes(strips, NT, kc, s) > budget) continue;
             if (kc * s > best) { best = kc * s; ksc = kc; nst = s; }
             break;
         }
@@ -217,23 +215,10 @@ bool choose_cfg(int n, bool cplx, int N, int n_gamma, int maxw, SpinCfg &c) {
         }
     }
     if (best < 0) return false;
-    // Two-half epilogue (k2_exchange.cuh): with at least two gamma blocks per tile the staging buffer holds the larger part
-    // only, and the ring is re-chosen with the shared memory that frees.  The tile shape above is chosen with the whole-tile
-    // staging buffer, so that it does not depend on this.
-    c.gH = c.gT;
-    if (c.gT >= 2 && nb <= 8 * WM) c.gH = std::min(c.gT - 1, (8 * WM) / nb);        // gH * nb <= 8 * WM: see do_half in k2_exchange
-    c.stg_strips = c.strips;
-    if (c.gH < c.gT) {
-        const int half0 = (c.gH * nb + 7) / 8, half1 = c.strips - (c.gH * nb) / 8;
-        c.stg_strips = std::max(half0, half1);
-        const size_t budget2 = c.ctas_per_sm == 1 ? (size_t)kMaxSmem : (size_t)(233472 / c.ctas_per_sm - 1024);
-        int ksc = 0, nst = 0;
-        if (choose_pipeline(c.strips, c.NT, ksteps, budget2, ksc, nst, c.stg_strips)) { c.ksc = ksc; c.nstages = nst; }
-    }
     c.nchunks = (ksteps + c.ksc - 1) / c.ksc;
     c.n_rt = (n_gamma + c.gT - 1) / c.gT;
     c.n_ct_max = (maxw + c.wT - 1) / c.wT;
-    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages, c.stg_strips);
+    c.k2_smem = k2_smem_bytes(c.strips, c.NT, c.ksc, c.nstages);
     k2_staging_shape(c.NT, c.H, c.LD2);
     c.layA = OperandLayout{n, c.strips, ksteps, c.gT, (long long)c.strips * ksteps * 32};
     c.layB = OperandLayout{n, c.NT, ksteps, c.wT, (long long)c.NT * ksteps * 32};
@@ -591,7 +576,6 @@ static int launch_k2(afqmc_ctx *ctx, int s, int w0, int count, cudaStream_t stre
     p2.ksteps = ctx->ksteps; p2.ksc = sc.ksc; p2.nchunks = sc.nchunks; p2.nstages = sc.nstages;
     p2.n_rt = sc.n_rt; p2.n_ct = (count + sc.wT - 1) / sc.wT;
     p2.n_gamma = ctx->n_gamma; p2.n_walkers = count; p2.maxw = ctx->maxw; p2.H = sc.H; p2.LD2 = sc.LD2;
-    p2.gH = sc.gH; p2.stg_strips = sc.stg_strips;
     p2.tbuf = sc.tbuf + (long long)w0 * ctx->n_gamma * 2; p2.xpart = sc.xpart + (long long)w0 * 2;
     const long long ntiles = (long long)p2.n_rt * p2.n_ct;
     const int grid = (int)std::min<long long>(ntiles, (long long)ctx->num_sms * sc.ctas_per_sm);

@@ -44,7 +44,6 @@ struct K2Params {
     int n_rt, n_ct;                // row tiles (gamma), column tiles (walkers)
     int n_gamma, n_walkers, maxw;
     int H, LD2;                    // staging buffer: row pair pitch LD2 (= 1 mod 16), odd-row offset H (= 8 mod 16)
-    int gH, stg_strips;            // gamma blocks of the first epilogue half (= gT: no split), strips the staging buffer holds
     double *tbuf;                  // [maxw][n_gamma][2]  traces of this spin
     double *xpart;                 // [n_rt][maxw][2]     exchange partial sums of this spin
 };
@@ -155,8 +154,8 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
     const uint32_t b_chunk_bytes = (uint32_t)P.ksc * NT * 256u;
     const uint32_t stage_bytes = a_chunk_bytes + b_chunk_bytes;
     unsigned char *stage_base = k2_smem;
-    double *staging = reinterpret_cast<double *>(k2_smem + (size_t)P.nstages * stage_bytes);   // [4*stg_strips][LD2]
-    double *red = staging + (size_t)P.stg_strips * 4 * LD2;                                     // [2][K2_MAX_WT][K2_MAX_WM][2]
+    double *staging = reinterpret_cast<double *>(k2_smem + (size_t)P.nstages * stage_bytes);   // [4*strips][LD2]
+    double *red = staging + (size_t)P.strips * 4 * LD2;                                         // [2][K2_MAX_WT][K2_MAX_WM][2]
     uint64_t *full_bar = reinterpret_cast<uint64_t *>(red + 2 * K2_MAX_WT * K2_MAX_WM * 2);
     uint64_t *empty_bar = full_bar + P.nstages;
     uint64_t *stg_full = empty_bar + P.nstages;          // every warp has parked its accumulators of this tile
@@ -233,7 +232,6 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
         constexpr int MM = decltype(mm_tag)::value;
         constexpr int MMA = MM > 0 ? MM : 1;
         uint32_t tpar = 0;                                      // parity of this CTA's tile counter
-        uint32_t epar = 0;                                      // parity of its epilogue-half counter (staging hand-offs)
         for (int rt = first_rt, ct = first_ct; rt < P.n_rt;) {
             double acc[MMA][NT][2];
             if constexpr (MM > 0) {
@@ -245,56 +243,41 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
             }
 
             // ------------------------------ epilogue ------------------------------
-            // The tile's gamma blocks are worked off in up to two halves ([0, gH) and [gH, gT)), so that the staging buffer
-            // holds half a tile and the shared memory it frees goes to the operand ring (a K loop with 15-20 k-steps in
-            // flight runs at 92-93 % of the DMMA peak, with 10 at 86 %: profiles/r2_k2_ablations.md).  Per half:
-            // Phase 1 (all warps): park the accumulators of the strips that reach into the half in the staging buffer, rows
-            // counted from the half's first strip (a strip on the boundary is parked in both halves), columns
-            // col = (plane*wT + wl)*n + j.  Rows are stored in pairs:
+            // Phase 1 (all warps): park the accumulators in the whole-tile staging buffer with the tile's own
+            // row/column numbering (row = g*nb + i, col = (plane*wT + wl)*n + j).  Rows are stored in pairs:
             //     element (row, col)  ->  (row >> 1) * LD2 + (row & 1) * H + col,     H = 8 mod 16,  LD2 = 1 mod 16,
             // which makes the fragment-order stores here, the row loads and the column loads of phase 2 all
-            // bank-conflict free (column loads 2-way when the block's first row is odd).
+            // bank-conflict free (column loads 2-way when g*n is odd).
 #if AFQMC_K2_ABLATE < 2
-            const int gtile = min(P.gT, P.n_gamma - rt * P.gT);                // valid gamma blocks of this tile
-            const int w0 = ct * P.wT;
-            const int wvalid = min(P.wT, P.n_walkers - w0);
-            const int planeoff = P.wT * n;
-            double *redp = red + tpar * (K2_MAX_WT * K2_MAX_WM * 2);          // double-buffered by tile parity
-            if (lane < K2_MAX_WT) { redp[(lane * K2_MAX_WM + warp) * 2] = 0.0; redp[(lane * K2_MAX_WM + warp) * 2 + 1] = 0.0; }
-            // The UPPER half [gH, gT) goes first: the host keeps gH * nb <= 8 * WM, so every second (third, ...) strip of a warp
-            // lies wholly in it and is dead afterwards; the LOWER half [0, gH) then parks first strips only.  (With the halves
-            // in a runtime loop all accumulators stay live through phase 2 and the kernel spills.)
-            auto do_half = [&](const int g_lo, const int g_hi, auto upper_tag) {
-                constexpr bool UPPER = decltype(upper_tag)::value;
-                const int row_lo = g_lo * P.nb, row_hi = g_hi * P.nb;       // rows [row_lo, row_hi) of the tile
-                const int sbase = row_lo >> 3;                                // first strip that reaches into the half
-                mbar_wait(stg_free, epar ^ 1u);                               // the previous half has been read out
-                if constexpr (MM > 0) {
+            mbar_wait(stg_free, tpar ^ 1u);                                    // previous tile has been read out
+            if constexpr (MM > 0) {
 #pragma unroll
-                    for (int m = 0; m < (UPPER ? MM : 1); ++m) {
-                        const int strip = warp + m * WM;
-                        if (UPPER ? (m > 0 || strip * 8 + 8 > row_lo) : (strip * 8 < row_hi)) {
-                            const int row = (strip - sbase) * 8 + (lane >> 2);
-                            double *dst = staging + (row >> 1) * LD2 + (row & 1) * H + 2 * (lane & 3);
+                for (int m = 0; m < MM; ++m) {
+                    const int row = (warp + m * WM) * 8 + (lane >> 2);
+                    double *dst = staging + (row >> 1) * LD2 + (row & 1) * H + 2 * (lane & 3);
 #pragma unroll
-                            for (int q = 0; q < NT; ++q) { dst[q * 8] = acc[m][q][0]; dst[q * 8 + 1] = acc[m][q][1]; }
-                        }
-                    }
+                    for (int q = 0; q < NT; ++q) { dst[q * 8] = acc[m][q][0]; dst[q * 8 + 1] = acc[m][q][1]; }
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(stg_full);
-                // Phase 2 (all warps, once the half is parked; the FP64 pipe is shared with the DMMAs, so these
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(stg_full);
+            {
+                // Phase 2 (all warps, once the whole tile is parked; the FP64 pipe is shared with the DMMAs, so these
                 // DFMAs are only cheap while no warp is feeding it DMMAs): one (gamma g, walker wl) block
                 // T = R + iI (n x n) per pass, lanes over j, loop over i:
                 //     Re x += R_ij R_ji - I_ij I_ji,    Im x += 2 R_ij I_ji   (sum_ij I_ij R_ji = sum_ij R_ij I_ji by relabelling),
                 //     t = sum_j T_jj.
-                // When the half has fewer blocks than warps, each block's i range is split into `rs` parts.
-                const int g0 = rt * P.gT + g_lo;
-                const int gvalid = max(0, min(g_hi, gtile) - g_lo);
+                // When the tile has fewer blocks than warps, each block's i range is split into `rs` parts.
+                const int g0 = rt * P.gT;
+                const int gvalid = min(P.gT, P.n_gamma - g0);
+                const int w0 = ct * P.wT;
+                const int wvalid = min(P.wT, P.n_walkers - w0);
+                const int planeoff = P.wT * n;
                 const int nblk = gvalid * wvalid;
-                const int rs = nblk > 0 ? max(1, WM / nblk) : 1;
-                const int roff = row_lo - sbase * 8;                          // staging row of the half's first block row
-                mbar_wait(stg_full, epar);
+                const int rs = max(1, WM / nblk);
+                double *redp = red + tpar * (K2_MAX_WT * K2_MAX_WM * 2);      // double-buffered by tile parity
+                if (lane < K2_MAX_WT) { redp[(lane * K2_MAX_WM + warp) * 2] = 0.0; redp[(lane * K2_MAX_WM + warp) * 2 + 1] = 0.0; }
+                mbar_wait(stg_full, tpar);
 #if AFQMC_K2_ABLATE == 1
                 for (int u = warp; u < 0; u += WM) {
 #else
@@ -303,7 +286,7 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
                     const int blk = u / rs, part = u - blk * rs;
                     const int g = blk / wvalid, wl = blk - g * wvalid;
                     const int i_lo = (part * n) / rs, i_hi = ((part + 1) * n) / rs;
-                    const int gn = roff + g * P.nb, cb = wl * n;
+                    const int gn = g * P.nb, cb = wl * n;
                     const bool cplx = P.cplx != 0;
                     // element T_ij = R + iI of the block, from the parked products C = Ltilde theta^T:
                     //   real Ltilde:     R = C[i][re j],                   I = C[i][im j]
@@ -354,21 +337,14 @@ __global__ void __maxnreg__(168) k2_exchange(const K2Params P) {   // blockDim <
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(stg_free);
-                epar ^= 1u;
-            };
-            if (P.gH < P.gT) {
-                do_half(P.gH, P.gT, std::true_type{});
-                do_half(0, P.gH, std::false_type{});
-            } else {
-                do_half(0, P.gT, std::true_type{});
-            }
-            if (warp == WM - 1) {                        // the lightest warp adds the per-warp shares in a fixed order
-                mbar_wait(stg_free, epar ^ 1u);          // the last half has been read out by every warp
-                if (lane < wvalid) {
-                    double sr = 0.0, si = 0.0;
-                    for (int q = 0; q < WM; ++q) { sr += redp[(lane * K2_MAX_WM + q) * 2]; si += redp[(lane * K2_MAX_WM + q) * 2 + 1]; }
-                    double *xp = P.xpart + ((long long)rt * P.maxw + w0 + lane) * 2;
-                    xp[0] = sr; xp[1] = si;
+                if (warp == WM - 1) {                    // the lightest warp adds the per-warp shares in a fixed order
+                    mbar_wait(stg_free, tpar);
+                    if (lane < wvalid) {
+                        double sr = 0.0, si = 0.0;
+                        for (int q = 0; q < WM; ++q) { sr += redp[(lane * K2_MAX_WM + q) * 2]; si += redp[(lane * K2_MAX_WM + q) * 2 + 1]; }
+                        double *xp = P.xpart + ((long long)rt * P.maxw + w0 + lane) * 2;
+                        xp[0] = sr; xp[1] = si;
+                    }
                 }
             }
 #else   // keep the products alive (ptxas would drop DMMAs whose results are never read)
